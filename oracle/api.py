@@ -1,0 +1,193 @@
+"""oracle/api.py — TEST INFRASTRUCTURE. ctypes front end of the CPU oracle (oracle/liboracle.so).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+Everything is numpy float64 in, float64 out; genes are float32 (reading G1).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+NPAR = 9
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.orc_lande_g.restype = C.c_double
+        _lib.orc_g_eff.restype = C.c_double
+        _lib.orc_chi2.restype = C.c_double
+        _lib.orc_lande_g.argtypes = [C.c_double] * 3
+        _lib.orc_g_eff.argtypes = [C.c_double] * 4
+    return _lib
+
+
+def hardware_threads():
+    return int(lib().orc_hardware_threads())
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def faddeeva(z):
+    z = np.asarray(z, dtype=np.complex128)
+    re, im = _f64(z.real.ravel()), _f64(z.imag.ravel())
+    wr, wi = np.empty_like(re), np.empty_like(im)
+    lib().orc_faddeeva(_p(re, C.c_double), _p(im, C.c_double), C.c_int64(re.size), _p(wr, C.c_double), _p(wi, C.c_double))
+    return (wr + 1j * wi).reshape(z.shape)
+
+
+def lande_g(S, L, J):
+    return lib().orc_lande_g(S, L, J)
+
+
+def g_eff(gl, Jl, gu, Ju):
+    return lib().orc_g_eff(gl, Jl, gu, Ju)
+
+
+def zeeman_pattern(lower, upper):
+    """lower/upper = (S, L, J). Returns (shift, weight, kind) arrays."""
+    cap = 256
+    sh, we, ki = np.zeros(cap), np.zeros(cap), np.zeros(cap, dtype=np.int32)
+    n = lib().orc_zeeman_pattern(*[C.c_double(x) for x in (*lower, *upper)], C.c_int(cap),
+                                 _p(sh, C.c_double), _p(we, C.c_double), _p(ki, C.c_int))
+    return sh[:n].copy(), we[:n].copy(), ki[:n].copy()
+
+
+class Lines:
+    """Line list for the oracle: list of dicts {lambda0, strength, shift[], weight[], kind[]} + lambda_ref."""
+
+    def __init__(self, lines, lambda_ref):
+        self.n = len(lines)
+        self.lambda_ref = float(lambda_ref)
+        self.lambda0 = _f64([l["lambda0"] for l in lines])
+        self.strength = _f64([l["strength"] for l in lines])
+        self.n_comp = _i32([len(l["shift"]) for l in lines])
+        self.shift = _f64(np.concatenate([np.asarray(l["shift"], dtype=np.float64) for l in lines]))
+        self.weight = _f64(np.concatenate([np.asarray(l["weight"], dtype=np.float64) for l in lines]))
+        self.kind = _i32(np.concatenate([np.asarray(l["kind"], dtype=np.int32) for l in lines]))
+
+    def args(self):
+        return [C.c_int(self.n), _p(self.lambda0, C.c_double), _p(self.strength, C.c_double), _p(self.n_comp, C.c_int),
+                _p(self.shift, C.c_double), _p(self.weight, C.c_double), _p(self.kind, C.c_int), C.c_double(self.lambda_ref)]
+
+
+def synth(params, lam, lines, mu=None, use_solve=False, threads=1):
+    params = _f64(params).reshape(-1, NPAR)
+    lam = _f64(lam)
+    P, L = params.shape[0], lam.size
+    mu_a = _f64(mu) if mu is not None else None
+    out = np.empty((P, 4, L))
+    lib().orc_synth(_p(params, C.c_double), _p(mu_a, C.c_double), C.c_int64(P), _p(lam, C.c_double), C.c_int(L),
+                    *lines.args(), C.c_int(int(use_solve)), C.c_int(threads), _p(out, C.c_double))
+    return out
+
+
+def absorption_matrix(p, lam, lines):
+    p = _f64(p)
+    out = np.empty(7)
+    lib().orc_absorption_matrix(_p(p, C.c_double), C.c_double(lam), *lines.args(), _p(out, C.c_double))
+    return out
+
+
+def chi2(obs, model, w, sigma, M=NPAR):
+    obs, model, w, sigma = _f64(obs), _f64(model), _f64(w), _f64(sigma)
+    L = obs.shape[-1]
+    return lib().orc_chi2(_p(obs, C.c_double), _p(model, C.c_double), C.c_int(L), _p(w, C.c_double), _p(sigma, C.c_double), C.c_int(M))
+
+
+def philox(seed, c0, c1, c2, c3):
+    out = np.zeros(4, dtype=np.uint32)
+    lib().orc_philox(C.c_uint64(seed), C.c_uint32(c0), C.c_uint32(c1), C.c_uint32(c2), C.c_uint32(c3), _p(out, C.c_uint32))
+    return out
+
+
+def philox_raw(ctr, key):
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32)
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    lib().orc_philox_raw(_p(ctr, C.c_uint32), _p(key, C.c_uint32), _p(out, C.c_uint32))
+    return out
+
+
+def decode(genes, cfg):
+    genes = np.ascontiguousarray(genes, dtype=np.float32).reshape(-1, NPAR)
+    out = np.empty(genes.shape)
+    lo, hi, lg = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"])
+    lib().orc_decode(_p(genes, C.c_float), C.c_int64(genes.shape[0]), _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(out, C.c_double))
+    return out
+
+
+def ga_init(N, pop, seed, pixel_base=0):
+    genes = np.empty((N, pop, NPAR), dtype=np.float32)
+    lib().orc_ga_init(C.c_int64(N), C.c_uint64(pixel_base), C.c_int(pop), C.c_uint64(seed), _p(genes, C.c_float))
+    return genes
+
+
+def _cfg_args(cfg):
+    ms = np.ascontiguousarray(cfg["mut_scale"], dtype=np.float32)
+    assert ms.size == cfg["generations"] + 1
+    keep = [ms]
+    return keep, [C.c_int(cfg["pop"]), C.c_int(cfg["generations"]), C.c_int(cfg["tournament_k"]),
+                  C.c_float(cfg["p_cross"]), C.c_float(cfg["p_mut"]), _p(ms, C.c_float)]
+
+
+def ga_step(genes, chi2v, t, cfg, seed, pixel_base=0):
+    genes = np.ascontiguousarray(genes, dtype=np.float32)
+    N, pop = genes.shape[0], genes.shape[1]
+    chi2v = _f64(chi2v)
+    out = np.empty_like(genes)
+    keep, a = _cfg_args(cfg)
+    per = _i32(cfg["periodic"])
+    lib().orc_ga_step(_p(genes, C.c_float), _p(chi2v, C.c_double), C.c_int64(N), C.c_uint64(pixel_base), C.c_int(t),
+                      *a, _p(per, C.c_int), C.c_uint64(seed), _p(out, C.c_float))
+    return out
+
+
+def ga_fitness(genes, obs, lam, lines, cfg, mu=None, threads=1):
+    genes = np.ascontiguousarray(genes, dtype=np.float32)
+    N, pop = genes.shape[0], genes.shape[1]
+    obs, lam = _f64(obs), _f64(lam)
+    mu_a = _f64(mu) if mu is not None else None
+    lo, hi, lg = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"])
+    w, sg = _f64(cfg["stokes_weight"]), _f64(cfg["sigma"])
+    out = np.empty((N, pop))
+    lib().orc_ga_fitness(_p(genes, C.c_float), _p(obs, C.c_double), _p(mu_a, C.c_double), C.c_int64(N), C.c_int(pop),
+                         _p(lam, C.c_double), C.c_int(lam.size), *lines.args(),
+                         _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(w, C.c_double), _p(sg, C.c_double),
+                         C.c_int(threads), _p(out, C.c_double))
+    return out
+
+
+def ga_invert(obs, lam, lines, cfg, seed, mask=None, mu=None, pixel_base=0, threads=1, want_trace=False):
+    """obs[N,4,L] -> dict(params[N,9], chi2[N], genes[N,9], trace[N,G+1] or None)."""
+    obs, lam = _f64(obs), _f64(lam)
+    N, L = obs.shape[0], lam.size
+    assert obs.shape == (N, 4, L)
+    mu_a = _f64(mu) if mu is not None else None
+    mask_a = np.ascontiguousarray(mask, dtype=np.uint8) if mask is not None else None
+    lo, hi, lg, per = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"]), _i32(cfg["periodic"])
+    w, sg = _f64(cfg["stokes_weight"]), _f64(cfg["sigma"])
+    keep, a = _cfg_args(cfg)
+    params, chi2v = np.empty((N, NPAR)), np.empty(N)
+    genes = np.full((N, NPAR), np.nan, dtype=np.float32)
+    trace = np.full((N, cfg["generations"] + 1), np.nan) if want_trace else None
+    lib().orc_ga_invert(_p(obs, C.c_double), _p(mask_a, C.c_ubyte), _p(mu_a, C.c_double), C.c_int64(N), C.c_uint64(pixel_base),
+                        _p(lam, C.c_double), C.c_int(L), *lines.args(), *a,
+                        _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(per, C.c_int),
+                        _p(w, C.c_double), _p(sg, C.c_double), C.c_uint64(seed), C.c_int(threads),
+                        _p(params, C.c_double), _p(chi2v, C.c_double), _p(genes, C.c_float), _p(trace, C.c_double))
+    return {"params": params, "chi2": chi2v, "genes": genes, "trace": trace}

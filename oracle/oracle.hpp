@@ -1,0 +1,86 @@
+// oracle/oracle.hpp — TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, double-precision CPU statement of what the GENESIS hot path computes
+// (Harker & Mighell, arxiv 1208.0302): Milne-Eddington forward synthesis of I,Q,U,V, the
+// chi-square merit (eq. 16) and the per-pixel genetic algorithm (Alg. 1).  It exists so that the
+// CUDA path under paper_1208_0302_b200/csrc has something independent to be compared with.
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// build, load or call it.  It shares no source, header, table or helper with the CUDA path.
+//
+// Citations are PAPER.md line numbers plus the equation they fall in;
+// "reading Fn/Gn" refers to the list of readings in DESIGN.md (taken from SURVEY.md §8(c)).
+//
+// Parity pins (tests/test_oracle_*.py, -m "not gpu"):
+//   faddeeva       pinned  (erfc / Dawson closed forms, scipy.special.wofz, ODE w' = -2zw + 2i/sqrt(pi))
+//   zeeman_pattern pinned  (Table 1 g_eff, 12 components for 6301.5, centre-of-gravity identity)
+//   synth          pinned  (B=0 and gamma=0 closed forms, 4x4 solve of eq. 12, symmetries, weak field)
+//   chi2           pinned  (expected value at truth, brute-force grid minimum)
+//   philox4x32_10  pinned  (published known-answer vectors of Salmon et al. 2011)
+//   ga             operators pinned by brute-force re-derivation in Python on tiny inputs and by
+//                  invariants; absolute recovery accuracy: PARITY UNPINNED (the paper prints no
+//                  reproducible recovery numbers, Table 4 PAPER.md:340-345 is for SOLIS data).
+#pragma once
+#include <complex>
+#include <cstdint>
+#include <vector>
+
+namespace orc {
+
+typedef std::complex<double> cplx;
+
+// ---- Faddeeva function w(z) = exp(-z^2) erfc(-iz), Im z > 0  (H = Re w, F = Im w; reading F3) ----
+cplx faddeeva(cplx z);
+
+// ---- Zeeman pattern in LS coupling ("full Zeeman pattern ... calculated at the start") ----
+struct Component { double shift; double weight; int kind; };   // kind: 0 = pi, -1 = sigma_blue, +1 = sigma_red
+double lande_g(double S, double L, double J);
+double g_eff(double gl, double Jl, double gu, double Ju);
+std::vector<Component> zeeman_pattern(double Sl, double Ll, double Jl, double Su, double Lu, double Ju);
+std::vector<Component> zeeman_triplet(double geff);
+
+// ---- Line table + model ----
+struct Line { double lambda0; double strength; std::vector<Component> comps; };
+struct Lines { std::vector<Line> lines; double lambda_ref; };
+
+// Parameter order (BASELINE config 0; differs from eq. 14):
+// [B (G), gamma (deg), chi (deg), eta0, dlambdaD (mA at lambda_ref), a, v_los (km/s), S0, S1]
+enum { P_B = 0, P_GAMMA, P_CHI, P_ETA0, P_DLD, P_A, P_VLOS, P_S0, P_S1, NPAR = 9 };
+
+// Absorption-matrix elements at one wavelength (eq. 8; reading F1/F2).
+struct Eta { double eI, eQ, eU, eV, rQ, rU, rV; };
+Eta absorption_matrix(const double* p, double lambda, const Lines& ln);
+
+// Unno-Rachkovsky solution, closed form (eq. 12-13, 15 PAPER.md:204-216; reading F6): out[4].
+void stokes_closed_form(const Eta& e, double S0, double muS1, double out[4]);
+// The same by building K and solving K x = e by Gaussian elimination (eq. 12 as printed).
+void stokes_by_solve(const Eta& e, double S0, double muS1, double out[4]);
+
+// Full profile: out[4][L].  use_solve selects the second path.
+void synth(const double* p, double mu, const double* lambda, int L, const Lines& ln, double* out, bool use_solve);
+
+// eq. 16, reading F11: chi2 = 1/nu * sum_s sum_j (w_s/sigma_s)^2 (O - M)^2, nu = 4L - M.
+double chi2(const double* obs, const double* model, int L, const double w[4], const double sigma[4], int M);
+
+// ---- Philox4x32-10 (Salmon et al. 2011), reading G0 ----
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+// ---- GA (Alg. 1; readings G0-G5) ----
+struct GaCfg {
+    int pop, generations, tournament_k;
+    float p_cross, p_mut;
+    std::vector<float> mut_scale;              // s_t for t = 0..generations (built by the caller, binary32)
+    double lo[NPAR], hi[NPAR];
+    int log_scale[NPAR], periodic[NPAR];
+    double w[4], sigma[4];
+    uint64_t seed;
+};
+double decode_gene(float g, double lo, double hi, int log_scale);
+// Next generation from (genes[pop][NPAR], chi2[pop]) at generation t >= 1 for global pixel id `pixel`.
+void ga_step(const float* genes, const double* chi2v, int t, uint64_t pixel, const GaCfg& c, float* out);
+void ga_init(uint64_t pixel, const GaCfg& c, float* genes);
+// Whole inversion of one pixel: obs[4][L] (double). Returns best decoded params and chi2;
+// if trace != nullptr it receives best chi2 per generation (generations+1 values).
+void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c,
+                     uint64_t pixel, double* best_params, double* best_chi2, float* best_genes, double* trace);
+
+}  // namespace orc
