@@ -1,0 +1,262 @@
+// me_api.cu — the C ABI of include/me.h: argument validation, descriptor construction (host), launches.
+#include <cmath>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "me_device.cuh"
+#include "me_launch.h"
+
+namespace {
+
+thread_local std::string g_cuda_err;
+
+int cuda_fail(cudaError_t e) {
+    g_cuda_err = cudaGetErrorString(e);
+    return ME_ERR_CUDA;
+}
+
+const double C_KMS = 299792.458;       // speed of light, km/s
+const double ZEEMAN = 4.66857e-13;     // e / (4 pi m_e c^2), A^-1 G^-1
+
+// Build the kernel-side synthesis descriptor from the caller's line list and wavelength grid.
+int build_synth_desc(const double* lambda, int L, const me_line_data* ld, me::SynthDesc& d) {
+    if (lambda == nullptr || ld == nullptr || ld->lines == nullptr) return ME_ERR_NULL;
+    if (L < 2 || L > ME_MAX_L) return ME_ERR_SHAPE;
+    if (ld->n_lines < 1 || ld->n_lines > ME_MAX_LINES) return ME_ERR_SHAPE;
+    if (ld->n_params == 11) return ME_ERR_UNSUPPORTED;
+    if (ld->n_params != ME_NPAR) return ME_ERR_SHAPE;
+    if (ld->nm_profile != nullptr) return ME_ERR_UNSUPPORTED;
+    if (!(ld->lambda_ref_A > 0.0)) return ME_ERR_RANGE;
+    std::memset(&d, 0, sizeof(d));
+    d.L = L; d.n_lines = ld->n_lines; d.all_triplets = 1;
+    int o = 0;
+    for (int l = 0; l < ld->n_lines; ++l) {
+        const me_line& ln = ld->lines[l];
+        if (ln.n_comp < 1 || ln.shift == nullptr || ln.weight == nullptr || ln.kind == nullptr) return ME_ERR_NULL;
+        if (o + ln.n_comp > ME_MAX_COMP) return ME_ERR_SHAPE;
+        if (!(ln.lambda0_A > 0.0) || !(ln.strength >= 0.0f)) return ME_ERR_RANGE;
+        me::LineDesc& q = d.line[l];
+        q.lam0_over_c = (float)(ln.lambda0_A / C_KMS);
+        q.dld_scale = (float)(1e-3 * ln.lambda0_A / ld->lambda_ref_A);
+        q.zeeman = (float)(ZEEMAN * ln.lambda0_A * ln.lambda0_A);
+        q.strength = ln.strength;
+        int cnt[3] = {0, 0, 0};
+        for (int kind = -1; kind <= 1; ++kind) {          // sorted [blue | pi | red]
+            q.kind_begin[kind + 1] = o;
+            for (int c = 0; c < ln.n_comp; ++c) {
+                if (ln.kind[c] < -1 || ln.kind[c] > 1) return ME_ERR_RANGE;
+                if (ln.kind[c] != kind) continue;
+                d.shift[o] = ln.shift[c]; d.weight[o] = ln.weight[c]; ++o; ++cnt[kind + 1];
+            }
+        }
+        q.kind_begin[3] = o;
+        const int b = q.kind_begin[0], p = q.kind_begin[1], r = q.kind_begin[2];
+        q.triplet = (cnt[0] == 1 && cnt[1] == 1 && cnt[2] == 1 && d.weight[b] == 1.0f && d.weight[p] == 1.0f &&
+                     d.weight[r] == 1.0f && d.shift[p] == 0.0f && d.shift[b] == -d.shift[r]) ? 1 : 0;
+        q.g = q.triplet ? d.shift[r] : 0.0f;
+        if (!q.triplet) d.all_triplets = 0;
+        for (int j = 0; j < L; ++j) d.off[l][j] = (float)(lambda[j] - ln.lambda0_A);   // formed in double, rounded once
+    }
+    d.n_comp = o;
+    return ME_OK;
+}
+
+int build_ga_desc(const ga_cfg* c, const float* sigma, int L, uint64_t seed, int64_t N, bool need_sigma, me::GaDesc& g) {
+    if (c == nullptr) return ME_ERR_NULL;
+    if (need_sigma && sigma == nullptr) return ME_ERR_NULL;
+    if (c->pop < 2 || c->pop > ME_MAX_POP) return ME_ERR_SHAPE;
+    if (c->generations < 0 || c->generations > ME_MAX_GEN) return ME_ERR_SHAPE;
+    if (c->tournament_k < 1 || c->tournament_k > 4) return ME_ERR_RANGE;
+    if (c->elite != 1) return ME_ERR_UNSUPPORTED;
+    if (!(c->p_cross >= 0.f && c->p_cross <= 1.f) || !(c->p_mut >= 0.f && c->p_mut <= 1.f)) return ME_ERR_RANGE;
+    if (c->pixel_id_base < 0 || N < 0 || (uint64_t)c->pixel_id_base + (uint64_t)N > 0x100000000ULL) return ME_ERR_RANGE;
+    std::memset(&g, 0, sizeof(g));
+    g.pop = c->pop; g.generations = c->generations; g.tournament_k = c->tournament_k;
+    g.p_cross = c->p_cross; g.p_mut = c->p_mut;
+    g.key0 = (uint32_t)(seed & 0xffffffffu); g.key1 = (uint32_t)(seed >> 32);
+    g.pixel_base = (uint32_t)c->pixel_id_base;
+    g.inv_nu = (float)(1.0 / (4.0 * L - ME_NPAR));
+    for (int s = 0; s < 4; ++s) {
+        double sg = need_sigma ? (double)sigma[s] : 1.0;
+        if (!(sg > 0.0) || !(c->stokes_weight[s] >= 0.f)) return ME_ERR_RANGE;
+        double w = (double)c->stokes_weight[s] / sg;
+        g.w2[s] = (float)(w * w);
+    }
+    for (int j = 0; j < ME_NPAR; ++j) {
+        if (!(c->lo[j] <= c->hi[j])) return ME_ERR_RANGE;
+        g.lo[j] = c->lo[j];
+        g.span[j] = (float)((double)c->hi[j] - (double)c->lo[j]);
+        g.log_scale[j] = c->log_scale[j] ? 1 : 0;
+        g.periodic[j] = c->periodic[j] ? 1 : 0;
+        if (g.log_scale[j]) {
+            if (!(c->lo[j] > 0.f)) return ME_ERR_RANGE;
+            g.log2ratio[j] = (float)std::log2((double)c->hi[j] / (double)c->lo[j]);
+        }
+    }
+    if (c->mut_scale_table != nullptr) {
+        for (int t = 0; t <= c->generations; ++t) g.mut_scale[t] = c->mut_scale_table[t];
+    } else {
+        if (!(c->mut_scale0 > 0.f) || !(c->mut_scale_end > 0.f)) return ME_ERR_RANGE;
+        const int G = c->generations > 0 ? c->generations : 1;
+        for (int t = 0; t <= c->generations; ++t)
+            g.mut_scale[t] = (float)((double)c->mut_scale0 * std::pow((double)c->mut_scale_end / (double)c->mut_scale0, (double)t / G));
+    }
+    return ME_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int me_version(void) { return 100; }
+
+const char* me_last_cuda_error(void) { return g_cuda_err.c_str(); }
+
+const char* me_strerror(int code) {
+    switch (code) {
+        case ME_OK: return "ok";
+        case ME_ERR_NULL: return "a required pointer is NULL";
+        case ME_ERR_SHAPE: return "a size is out of range";
+        case ME_ERR_RANGE: return "a value is out of range";
+        case ME_ERR_UNSUPPORTED: return "not implemented in this build";
+        case ME_ERR_CUDA: return "CUDA runtime error (see me_last_cuda_error)";
+        default: return "unknown error code";
+    }
+}
+
+int me_synth(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
+             const me_line_data* line_data, float* out_stokes,
+             const float* obs_ref, const float* w_over_sigma, float* out_chi2, void* stream) {
+    if (P < 0) return ME_ERR_SHAPE;
+    if (out_stokes == nullptr && out_chi2 == nullptr) return ME_ERR_NULL;
+    if (out_chi2 != nullptr && (obs_ref == nullptr || w_over_sigma == nullptr)) return ME_ERR_NULL;
+    me::SynthDesc sd;
+    int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
+    if (rc != ME_OK) return rc;
+    if (P == 0) return ME_OK;
+    if (params == nullptr) return ME_ERR_NULL;
+    float w2[4] = {0, 0, 0, 0};
+    if (out_chi2 != nullptr)
+        for (int s = 0; s < 4; ++s) {
+            if (!(w_over_sigma[s] >= 0.f)) return ME_ERR_RANGE;
+            w2[s] = w_over_sigma[s] * w_over_sigma[s];
+        }
+    cudaError_t e = me::launch_synth(sd, params, mu, P, out_stokes, obs_ref, w2, (float)(1.0 / (4.0 * L - ME_NPAR)),
+                                     out_chi2, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sigma,
+              const double* lambda_grid_A, int L, const me_line_data* line_data, const ga_cfg* cfg, uint64_t seed,
+              float* out_params, float* out_chi2, void* stream) {
+    me::SynthDesc sd; me::GaDesc gd;
+    int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
+    if (rc != ME_OK) return rc;
+    rc = build_ga_desc(cfg, sigma, L, seed, N, true, gd);
+    if (rc != ME_OK) return rc;
+    if (N == 0) return ME_OK;
+    if (obs == nullptr || out_params == nullptr || out_chi2 == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_ga_invert(sd, gd, obs, mask, cfg->mu, N, out_params, out_chi2, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int ga_fitness(const float* genes, const float* obs, int64_t N, const float* sigma, const double* lambda_grid_A, int L,
+               const me_line_data* line_data, const ga_cfg* cfg, float* chi2_out, void* stream) {
+    me::SynthDesc sd; me::GaDesc gd;
+    int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
+    if (rc != ME_OK) return rc;
+    rc = build_ga_desc(cfg, sigma, L, 0, N, true, gd);
+    if (rc != ME_OK) return rc;
+    if (N == 0) return ME_OK;
+    if (genes == nullptr || obs == nullptr || chi2_out == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_ga_fitness(sd, gd, genes, obs, cfg->mu, N, chi2_out, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int ga_step(const float* genes_in, const float* chi2_in, int64_t N, int generation, const ga_cfg* cfg, int n_params,
+            uint64_t seed, float* genes_out, void* stream) {
+    if (n_params == 11) return ME_ERR_UNSUPPORTED;
+    if (n_params != ME_NPAR) return ME_ERR_SHAPE;
+    me::GaDesc gd;
+    int rc = build_ga_desc(cfg, nullptr, 4, seed, N, false, gd);
+    if (rc != ME_OK) return rc;
+    if (generation < 1 || generation > cfg->generations) return ME_ERR_RANGE;
+    if (N == 0) return ME_OK;
+    if (genes_in == nullptr || chi2_in == nullptr || genes_out == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_ga_step(gd, genes_in, chi2_in, N, generation, genes_out, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int ga_init(int64_t N, const ga_cfg* cfg, uint64_t seed, float* genes_out, void* stream) {
+    me::GaDesc gd;
+    int rc = build_ga_desc(cfg, nullptr, 4, seed, N, false, gd);
+    if (rc != ME_OK) return rc;
+    if (N == 0) return ME_OK;
+    if (genes_out == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_ga_init(gd, N, genes_out, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int me_philox_many(uint64_t seed, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3, int64_t n, uint32_t* out,
+                   void* stream) {
+    if (n < 0) return ME_ERR_SHAPE;
+    if (n == 0) return ME_OK;
+    if (out == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_philox((uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), c0_base, c1, c2, c3, n, out,
+                                      (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int me_philox(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t out[4]) {
+    if (out == nullptr) return ME_ERR_NULL;
+    uint32_t* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, 16);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = me::launch_philox((uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), c0, c1, c2, c3, 1, d, nullptr);
+    if (e == cudaSuccess) e = cudaMemcpy(out, d, 16, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int me_faddeeva(const float* v, const float* a, int64_t n, float* H, float* F, void* stream) {
+    if (n < 0) return ME_ERR_SHAPE;
+    if (n == 0) return ME_OK;
+    if (v == nullptr || a == nullptr || H == nullptr || F == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_faddeeva(v, a, n, H, F, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+// Zeeman pattern in LS coupling: Lande factors, shifts g_l M_l - g_u M_u, dipole strengths per Delta M.
+int me_zeeman_pattern(double S_lo, double L_lo, double J_lo, double S_up, double L_up, double J_up,
+                      int cap, float* shift, float* weight, int8_t* kind) {
+    if (cap > 0 && (shift == nullptr || weight == nullptr || kind == nullptr)) return ME_ERR_NULL;
+    const double dJd = J_up - J_lo;
+    const int dJ = (int)std::lround(dJd);
+    if (J_lo < 0 || J_up < 0 || std::fabs(dJd - dJ) > 1e-9 || dJ < -1 || dJ > 1 || (J_lo == 0 && J_up == 0)) return ME_ERR_RANGE;
+    auto lande = [](double S, double L, double J) {
+        return J == 0.0 ? 0.0 : 1.5 + (S * (S + 1) - L * (L + 1)) / (2 * J * (J + 1));
+    };
+    const double gl = lande(S_lo, L_lo, J_lo), gu = lande(S_up, L_up, J_up);
+    int n = 0;
+    for (int q = 1; q >= -1; --q) {                       // q = M_up - M_lo: +1 -> sigma_blue, 0 -> pi, -1 -> sigma_red
+        std::vector<double> sh, st;
+        double tot = 0;
+        const int nM = (int)std::lround(2 * J_lo) + 1;
+        for (int k = 0; k < nM; ++k) {
+            const double M = -J_lo + k, Mu = M + q;
+            if (std::fabs(Mu) > J_up + 1e-9) continue;
+            double s;
+            if (dJ == 0)      s = q == 0 ? M * M : (q == 1 ? (J_lo - M) * (J_lo + M + 1) : (J_lo + M) * (J_lo - M + 1));
+            else if (dJ == 1) s = q == 0 ? (J_lo + 1) * (J_lo + 1) - M * M : (q == 1 ? (J_lo + M + 1) * (J_lo + M + 2) : (J_lo - M + 1) * (J_lo - M + 2));
+            else              s = q == 0 ? J_lo * J_lo - M * M : (q == 1 ? (J_lo - M) * (J_lo - M - 1) : (J_lo + M) * (J_lo + M - 1));
+            if (s <= 0) continue;
+            sh.push_back(gl * M - gu * Mu); st.push_back(s); tot += s;
+        }
+        for (size_t c = 0; c < sh.size(); ++c, ++n)
+            if (n < cap) { shift[n] = (float)sh[c]; weight[n] = (float)(st[c] / tot); kind[n] = (int8_t)(-q); }
+    }
+    return n;
+}
+
+}  // extern "C"

@@ -1,0 +1,389 @@
+// me_kernels.cu — CUDA kernels of libme_b200.so (sm_100a) and their launchers.
+//
+//   ga_invert_kernel   CTA = one pixel, thread = one individual; the whole GA of Alg. 1 runs
+//                      on-chip: observation staged once in shared memory, population double-buffered in shared
+//                      memory, fitness (synthesis + eq. 16) accumulated in registers over a serial wavelength loop.
+//   me_synth_kernel    warp = one parameter vector, lane = wavelength (coalesced [P,4,L] stores), optional chi2.
+//   ga_fitness_kernel / ga_step_kernel / ga_init_kernel / philox_kernel / faddeeva_kernel: test hooks.
+//
+// The paper's own mapping (block = individual, thread = wavelength, GA on the host with per-generation PCIe
+// transfers) is prior art for a Tesla C1060 and is deliberately not followed:
+// see DESIGN.md "What differs from the paper".
+#include "me_device.cuh"
+#include "me_launch.h"
+
+namespace me {
+
+// ------------------------------------------------------------------------------------------------------------
+// Fitness of one individual held in registers: decode -> per-individual constants -> wavelength loop.
+// obs_s: shared memory, [L] float4 = (I,Q,U,V) at each wavelength (broadcast reads, conflict-free).
+// ------------------------------------------------------------------------------------------------------------
+template <int NL, bool TRIPLET>
+__device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
+                                         const float4* obs_s) {
+    float p[ME_NPAR];
+#pragma unroll
+    for (int j = 0; j < ME_NPAR; ++j) p[j] = decode_gene(g[j], gd, j);
+    Individual<NL> ind;
+    setup_individual<NL>(ind, p, mu, sd);
+    float aI = 0.f, aQ = 0.f, aU = 0.f, aV = 0.f;
+    const int L = sd.L;
+    for (int j = 0; j < L; ++j) {
+        float I, Q, U, V;
+        stokes_at<NL, TRIPLET>(ind, sd, j, I, Q, U, V);
+        const float4 o = obs_s[j];
+        const float dI = o.x - I, dQ = o.y - Q, dU = o.z - U, dV = o.w - V;
+        aI = fmaf(dI, dI, aI); aQ = fmaf(dQ, dQ, aQ); aU = fmaf(dU, dU, aU); aV = fmaf(dV, dV, aV);
+    }
+    float chi2 = gd.inv_nu * fmaf(gd.w2[0], aI, fmaf(gd.w2[1], aQ, fmaf(gd.w2[2], aU, gd.w2[3] * aV)));
+    if (!(chi2 < __int_as_float(0x7f800000))) chi2 = __int_as_float(0x7f800000);   // NaN / Inf -> +Inf (reading G4)
+    return chi2;
+}
+
+// Stage obs[n] ([4][L] in HBM, rows contiguous => coalesced) into shared memory as [L] float4.
+__device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int L, int tid, int nthreads) {
+    for (int k = tid; k < 4 * L; k += nthreads) {
+        const int s = k / L, j = k - s * L;
+        obs_s[4 * j + s] = __ldg(obs_n + k);
+    }
+}
+
+// Block-wide argmin of (value, index) with ties -> lowest index. Values must be >= 0 or +Inf.
+// scratch: 2 * 32 words of shared memory. Every thread returns the same (value, index).
+__device__ __forceinline__ void block_argmin(float v, int idx, uint32_t* scratch, float& vmin, int& imin) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    uint32_t bits = __float_as_uint(v);
+    uint32_t m = __reduce_min_sync(0xffffffffu, bits);
+    uint32_t i = __reduce_min_sync(0xffffffffu, bits == m ? (uint32_t)idx : 0xffffffffu);
+    if (lane == 0) { scratch[warp] = m; scratch[32 + warp] = i; }
+    __syncthreads();
+    const uint32_t mb = lane < nwarps ? scratch[lane] : 0xffffffffu;
+    const uint32_t ib = lane < nwarps ? scratch[32 + lane] : 0xffffffffu;
+    m = __reduce_min_sync(0xffffffffu, mb);
+    i = __reduce_min_sync(0xffffffffu, mb == m ? ib : 0xffffffffu);
+    vmin = __uint_as_float(m);
+    imin = (int)i;
+    __syncthreads();          // scratch may be reused by the next call
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// The fused GA inversion kernel.
+// Dynamic shared memory: obs_s [L] float4 | genes [2][pop][9] | chi2 [2][pop] | scratch [64]
+// ------------------------------------------------------------------------------------------------------------
+template <int NL, bool TRIPLET, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
+                 const float* __restrict__ obs, const uint8_t* __restrict__ mask, const float* __restrict__ mu_arr,
+                 int64_t N, float* __restrict__ out_params, float* __restrict__ out_chi2) {
+    extern __shared__ float4 smem4[];
+    const int L = sd.L, pop = gd.pop;
+    float* obs_s = reinterpret_cast<float*>(smem4);
+    float* genes_s = obs_s + 4 * L;
+    float* chi2_s = genes_s + 2 * pop * ME_NPAR;
+    uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + 2 * pop);
+    const int tid = threadIdx.x;
+    const float INF = __int_as_float(0x7f800000);
+
+    for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
+        if (mask != nullptr && mask[n] == 0) {
+            const float qnan = __int_as_float(0x7fc00000);
+            if (tid < ME_NPAR) out_params[n * ME_NPAR + tid] = qnan;
+            if (tid == 0) out_chi2[n] = qnan;
+            continue;
+        }
+        const uint32_t pixel = gd.pixel_base + (uint32_t)n;
+        const float mu = mu_arr != nullptr ? __ldg(mu_arr + n) : 1.0f;
+        __syncthreads();                                   // previous pixel's shared memory is no longer read
+        stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
+
+        // generation 0 (reading G2)
+        float g[ME_NPAR];
+        float f = INF;
+        int cur = 0;
+        const bool alive = tid < pop;
+        if (alive) {
+            init_genes(g, pixel, (uint32_t)tid, gd);
+#pragma unroll
+            for (int j = 0; j < ME_NPAR; ++j) genes_s[tid * ME_NPAR + j] = g[j];
+        }
+        __syncthreads();
+        if (alive) { f = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s)); chi2_s[tid] = f; }
+        __syncthreads();
+
+        for (int t = 1; t <= gd.generations; ++t) {
+            float fe; int ie;
+            block_argmin(f, tid, scratch, fe, ie);         // elite of generation t-1
+            const float* gprev = genes_s + cur * pop * ME_NPAR;
+            const float* fprev = chi2_s + cur * pop;
+            float* gnext = genes_s + (cur ^ 1) * pop * ME_NPAR;
+            if (alive) {
+                if (tid == 0) {
+#pragma unroll
+                    for (int j = 0; j < ME_NPAR; ++j) g[j] = gprev[ie * ME_NPAR + j];
+                    f = fe;                                // carried, not re-evaluated (reading G3)
+                } else {
+                    make_child(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
+                    f = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
+                }
+#pragma unroll
+                for (int j = 0; j < ME_NPAR; ++j) gnext[tid * ME_NPAR + j] = g[j];
+                chi2_s[(cur ^ 1) * pop + tid] = f;
+            }
+            cur ^= 1;
+            __syncthreads();
+        }
+
+        float fe; int ie;
+        block_argmin(f, tid, scratch, fe, ie);             // reading G5
+        if (tid == ie) {
+#pragma unroll
+            for (int j = 0; j < ME_NPAR; ++j) out_params[n * ME_NPAR + j] = decode_gene(g[j], gd, j);
+            out_chi2[n] = f;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// me_synth: warp = parameter vector, lane = wavelength.  out_stokes[P,4,L]: each (vector, Stokes) row is
+// written as consecutive 128-byte warp stores.  chi2 (optional) is reduced with warp shuffles.
+// ------------------------------------------------------------------------------------------------------------
+template <int NL, bool TRIPLET>
+__global__ void __launch_bounds__(256)
+me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
+                int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
+                float w2I, float w2Q, float w2U, float w2V, float inv_nu, float* __restrict__ out_chi2) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warp0 = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int64_t nwarps = (int64_t)gridDim.x * (blockDim.x >> 5);
+    const int L = sd.L;
+    for (int64_t v = warp0; v < P; v += nwarps) {
+        float p[ME_NPAR];
+#pragma unroll
+        for (int j = 0; j < ME_NPAR; ++j) p[j] = __ldg(params + v * ME_NPAR + j);
+        const float mu = mu_arr != nullptr ? __ldg(mu_arr + v) : 1.0f;
+        Individual<NL> ind;
+        setup_individual<NL>(ind, p, mu, sd);
+        float acc = 0.f;
+        float* o = out_stokes != nullptr ? out_stokes + v * 4 * (int64_t)L : nullptr;
+        for (int j = lane; j < L; j += 32) {
+            float I, Q, U, V;
+            stokes_at<NL, TRIPLET>(ind, sd, j, I, Q, U, V);
+            if (o != nullptr) {
+                __stcs(o + j, I); __stcs(o + L + j, Q); __stcs(o + 2 * L + j, U); __stcs(o + 3 * L + j, V);
+            }
+            if (out_chi2 != nullptr) {
+                const float dI = __ldg(obs_ref + j) - I, dQ = __ldg(obs_ref + L + j) - Q;
+                const float dU = __ldg(obs_ref + 2 * L + j) - U, dV = __ldg(obs_ref + 3 * L + j) - V;
+                acc = fmaf(w2I * dI, dI, acc); acc = fmaf(w2Q * dQ, dQ, acc);
+                acc = fmaf(w2U * dU, dU, acc); acc = fmaf(w2V * dV, dV, acc);
+            }
+        }
+        if (out_chi2 != nullptr) {
+#pragma unroll
+            for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+            if (lane == 0) out_chi2[v] = acc * inv_nu;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Test hooks
+// ------------------------------------------------------------------------------------------------------------
+template <int NL, bool TRIPLET, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+ga_fitness_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
+                  const float* __restrict__ genes, const float* __restrict__ obs, const float* __restrict__ mu_arr,
+                  int64_t N, float* __restrict__ chi2_out) {
+    extern __shared__ float4 smem4[];
+    float* obs_s = reinterpret_cast<float*>(smem4);
+    const int L = sd.L, pop = gd.pop, tid = threadIdx.x;
+    for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
+        __syncthreads();
+        stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
+        __syncthreads();
+        if (tid < pop) {
+            float g[ME_NPAR];
+#pragma unroll
+            for (int j = 0; j < ME_NPAR; ++j) g[j] = genes[(n * pop + tid) * ME_NPAR + j];
+            const float mu = mu_arr != nullptr ? __ldg(mu_arr + n) : 1.0f;
+            chi2_out[n * pop + tid] = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
+        }
+    }
+}
+
+// One generation from given genes and given fitness (shared: genes [pop][9] | chi2 [pop] | scratch [64]).
+__global__ void ga_step_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ genes_in,
+                               const float* __restrict__ chi2_in, int64_t N, int t, float* __restrict__ genes_out) {
+    extern __shared__ float4 smem4[];
+    const int pop = gd.pop, tid = threadIdx.x;
+    float* genes_s = reinterpret_cast<float*>(smem4);
+    float* chi2_s = genes_s + pop * ME_NPAR;
+    uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + pop);
+    const float INF = __int_as_float(0x7f800000);
+    for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
+        __syncthreads();
+        for (int k = tid; k < pop * ME_NPAR; k += blockDim.x) genes_s[k] = genes_in[n * pop * ME_NPAR + k];
+        float f = INF;
+        if (tid < pop) {
+            f = chi2_in[n * pop + tid];
+            if (!(f < INF)) f = INF;
+            chi2_s[tid] = f;
+        }
+        __syncthreads();
+        float fe; int ie;
+        block_argmin(f, tid, scratch, fe, ie);
+        if (tid < pop) {
+            float g[ME_NPAR];
+            if (tid == 0) {
+#pragma unroll
+                for (int j = 0; j < ME_NPAR; ++j) g[j] = genes_s[ie * ME_NPAR + j];
+            } else {
+                make_child(g, genes_s, chi2_s, gd.pixel_base + (uint32_t)n, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
+            }
+#pragma unroll
+            for (int j = 0; j < ME_NPAR; ++j) genes_out[(n * pop + tid) * ME_NPAR + j] = g[j];
+        }
+    }
+}
+
+__global__ void ga_init_kernel(const __grid_constant__ GaDesc gd, int64_t N, float* __restrict__ genes_out) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N * gd.pop) return;
+    const int64_t n = k / gd.pop;
+    const int i = (int)(k - n * gd.pop);
+    float g[ME_NPAR];
+    init_genes(g, gd.pixel_base + (uint32_t)n, (uint32_t)i, gd);
+#pragma unroll
+    for (int j = 0; j < ME_NPAR; ++j) genes_out[k * ME_NPAR + j] = g[j];
+}
+
+__global__ void philox_kernel(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3,
+                              int64_t n, uint4* __restrict__ out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = philox4x32_10(c0_base + (uint32_t)i, c1, c2, c3, k0, k1);
+}
+
+__global__ void faddeeva_kernel(const float* __restrict__ v, const float* __restrict__ a, int64_t n,
+                                float* __restrict__ H, float* __restrict__ F) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float wr, wi;
+    faddeeva32(v[i], fad_const(a[i]), wr, wi);
+    H[i] = wr; F[i] = wi;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Launchers
+// ------------------------------------------------------------------------------------------------------------
+static inline unsigned grid_for(int64_t n) { return (unsigned)(n < 0x7fffffffLL ? n : 0x7fffffffLL); }
+
+static inline size_t ga_smem_bytes(int L, int pop) {
+    return (size_t)16 * L + (size_t)2 * pop * ME_NPAR * 4 + (size_t)2 * pop * 4 + 64 * 4;
+}
+
+template <int NL, bool TRIPLET, int THREADS, int MINB>
+static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask,
+                                      const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
+    auto k = ga_invert_kernel<NL, TRIPLET, THREADS, MINB>;
+    const size_t smem = ga_smem_bytes(sd.L, gd.pop);
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k<<<grid_for(N), THREADS, smem, st>>>(sd, gd, obs, mask, mu, N, out_params, out_chi2);
+    return cudaGetLastError();
+}
+
+template <int NL, bool TRIPLET, int THREADS, int MINB>
+static cudaError_t launch_ga_fitness_t(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs,
+                                       const float* mu, int64_t N, float* chi2_out, cudaStream_t st) {
+    auto k = ga_fitness_kernel<NL, TRIPLET, THREADS, MINB>;
+    const size_t smem = (size_t)16 * sd.L;
+    k<<<grid_for(N), THREADS, smem, st>>>(sd, gd, genes, obs, mu, N, chi2_out);
+    return cudaGetLastError();
+}
+
+// (pop -> block size, min blocks/SM) keeps the fitness loop at <= 128 registers/thread where the block allows it.
+#define ME_DISPATCH_THREADS(FN, NL, TR, ...)                                                       \
+    do {                                                                                            \
+        const int pop_ = gd.pop;                                                                    \
+        if (pop_ <= 64) return FN<NL, TR, 64, 8>(__VA_ARGS__);                                      \
+        if (pop_ <= 128) return FN<NL, TR, 128, 4>(__VA_ARGS__);                                    \
+        if (pop_ <= 256) return FN<NL, TR, 256, 2>(__VA_ARGS__);                                    \
+        if (pop_ <= 512) return FN<NL, TR, 512, 1>(__VA_ARGS__);                                    \
+        return FN<NL, TR, 1024, 1>(__VA_ARGS__);                                                    \
+    } while (0)
+
+#define ME_DISPATCH(FN, ...)                                                                        \
+    do {                                                                                            \
+        if (sd.all_triplets) {                                                                      \
+            if (sd.n_lines == 1) ME_DISPATCH_THREADS(FN, 1, true, __VA_ARGS__);                     \
+            if (sd.n_lines == 2) ME_DISPATCH_THREADS(FN, 2, true, __VA_ARGS__);                     \
+            ME_DISPATCH_THREADS(FN, ME_MAX_LINES, true, __VA_ARGS__);                               \
+        } else {                                                                                    \
+            if (sd.n_lines == 1) ME_DISPATCH_THREADS(FN, 1, false, __VA_ARGS__);                    \
+            if (sd.n_lines == 2) ME_DISPATCH_THREADS(FN, 2, false, __VA_ARGS__);                    \
+            ME_DISPATCH_THREADS(FN, ME_MAX_LINES, false, __VA_ARGS__);                              \
+        }                                                                                           \
+    } while (0)
+
+cudaError_t launch_ga_invert(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask, const float* mu,
+                             int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
+    ME_DISPATCH(launch_ga_invert_t, sd, gd, obs, mask, mu, N, out_params, out_chi2, st);
+}
+
+cudaError_t launch_ga_fitness(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs, const float* mu,
+                              int64_t N, float* chi2_out, cudaStream_t st) {
+    ME_DISPATCH(launch_ga_fitness_t, sd, gd, genes, obs, mu, N, chi2_out, st);
+}
+
+cudaError_t launch_ga_step(const GaDesc& gd, const float* genes_in, const float* chi2_in, int64_t N, int t,
+                           float* genes_out, cudaStream_t st) {
+    const int threads = ((gd.pop + 31) / 32) * 32;
+    const size_t smem = (size_t)gd.pop * ME_NPAR * 4 + (size_t)gd.pop * 4 + 64 * 4;
+    ga_step_kernel<<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ga_init(const GaDesc& gd, int64_t N, float* genes_out, cudaStream_t st) {
+    const int64_t total = N * gd.pop;
+    ga_init_kernel<<<grid_for((total + 255) / 256), 256, 0, st>>>(gd, N, genes_out);
+    return cudaGetLastError();
+}
+
+template <int NL, bool TRIPLET>
+static cudaError_t launch_synth_t(const SynthDesc& sd, const float* params, const float* mu, int64_t P, float* out_stokes,
+                                  const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, cudaStream_t st) {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int64_t blocks_needed = (P + 7) / 8;                       // 8 warps per block
+    const int64_t cap = (int64_t)sms * 8;                            // persistent grid: 8 resident blocks per SM
+    const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
+    me_synth_kernel<NL, TRIPLET><<<grid, 256, 0, st>>>(sd, params, mu, P, out_stokes, obs_ref, w2[0], w2[1], w2[2], w2[3],
+                                                       inv_nu, out_chi2);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* mu, int64_t P, float* out_stokes,
+                         const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, cudaStream_t st) {
+    if (sd.all_triplets) {
+        if (sd.n_lines == 1) return launch_synth_t<1, true>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
+        if (sd.n_lines == 2) return launch_synth_t<2, true>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
+        return launch_synth_t<ME_MAX_LINES, true>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
+    }
+    if (sd.n_lines == 1) return launch_synth_t<1, false>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
+    if (sd.n_lines == 2) return launch_synth_t<2, false>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
+    return launch_synth_t<ME_MAX_LINES, false>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
+}
+
+cudaError_t launch_philox(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3, int64_t n,
+                          uint32_t* out, cudaStream_t st) {
+    philox_kernel<<<grid_for((n + 255) / 256), 256, 0, st>>>(k0, k1, c0_base, c1, c2, c3, n, reinterpret_cast<uint4*>(out));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_faddeeva(const float* v, const float* a, int64_t n, float* H, float* F, cudaStream_t st) {
+    faddeeva_kernel<<<grid_for((n + 255) / 256), 256, 0, st>>>(v, a, n, H, F);
+    return cudaGetLastError();
+}
+
+}  // namespace me

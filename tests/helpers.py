@@ -28,4 +28,5 @@ def make_obs(cfg, n, seed_truth=W.SEED_TRUTH, seed_noise=W.SEED_NOISE, mu=None, 
     ln = oracle_lines(cfg["lines"], cfg["triplets"])
     clean = orc.synth(truth, cfg["lam"], ln, mu=mu, threads=threads)
     obs = clean + W.draw_noise(clean.shape, cfg["sigma"], seed=seed_noise)
+    obs = obs.astype(np.float32).astype(np.float64)       # the cube is binary32 ([N,4,L] f32): both sides read the same values
     return truth, obs, ln

@@ -1,0 +1,169 @@
+"""GPU parity tests: the CUDA path (through the C ABI via paper_1208_0302_b200.binding) against the CPU oracle,
+element by element on the same seeded inputs.  Run on the B200 box: pytest -m gpu.
+
+Tolerances:
+  forward synthesis   max |dStokes| / I_c <= 2e-5                      (north_star)
+  fused fitness       |dchi2| / chi2 <= 2e-4 (typically 1e-5)          (SURVEY.md par. 7: trajectory parity needs <~ 1e-4)
+  GA discrete state   bit-exact given the same fitness                 (readings G0-G3)
+  full inversion      median chi2 within 1 %, median |dB|,|dgamma|,|dchi|,|dv| within 5 % of the oracle's (north_star)
+"""
+import os
+
+import numpy as np
+import pytest
+
+from helpers import make_obs, oracle_lines
+from oracle import api as orc
+from paper_1208_0302_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+NTHREADS = max(1, (os.cpu_count() or 1))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1208_0302_b200 import binding, build
+    build.build()
+    binding.lib()
+    assert torch.cuda.is_available()
+    return binding
+
+
+def dev(a, dtype=np.float32):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
+
+
+# ---------------------------------------------------------------------------------------------------- RNG
+def test_philox_device_bit_exact(B):
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")):
+        line = line.split("#")[0].split()
+        if not line:
+            continue
+        v = [int(x, 16) for x in line]
+        got = B.me_philox(v[4] | (v[5] << 32), *v[0:4])
+        assert list(got) == v[6:10]
+    n = 20000
+    seed = 0x1234567890ABCDEF
+    got = B.me_philox_many(seed, 4294967000, 7, 9, 2, n).cpu().numpy().view(np.uint32)   # c0 wraps past 2^32
+    for i in list(range(0, 600)) + list(range(n - 200, n)):
+        assert tuple(got[i]) == tuple(orc.philox(seed, (4294967000 + i) & 0xffffffff, 7, 9, 2))
+    assert len({tuple(r) for r in got}) == n
+
+
+# ---------------------------------------------------------------------------------------------------- Faddeeva
+def test_faddeeva_device_vs_oracle(B):
+    rng = np.random.default_rng(5)
+    n = 400000
+    a = rng.uniform(0.01, 0.5, n).astype(np.float32)
+    v = np.concatenate([rng.uniform(-8, 8, n // 2), rng.uniform(-90, 90, n - n // 2)]).astype(np.float32)
+    v[:7] = [0.0, 5.5, -5.5, 5.4999, 1e-6, 89.0, -0.5]
+    H, F = B.me_faddeeva(dev(v), dev(a))
+    H, F = H.cpu().numpy().astype(np.float64), F.cpu().numpy().astype(np.float64)
+    ref = orc.faddeeva(v.astype(np.float64) + 1j * a.astype(np.float64))
+    assert np.max(np.abs(H - ref.real)) < 1.5e-6 and np.max(np.abs(F - ref.imag)) < 1.5e-6
+    wing = (v.astype(np.float64) ** 2 + a.astype(np.float64) ** 2) >= 5.6 ** 2
+    assert np.max(np.abs(H - ref.real)[wing] / ref.real[wing]) < 3e-6      # no cancellation in the wing form
+    assert np.max(np.abs(F - ref.imag)[wing] / np.abs(ref.imag[wing])) < 2e-6
+    # where H matters for the profiles (H*eta ~ 1): relative accuracy in the core
+    core = ~wing & (ref.real > 1e-3)
+    assert np.max(np.abs(H - ref.real)[core] / ref.real[core]) < 5e-4
+
+
+# ---------------------------------------------------------------------------------------------------- synthesis
+SYNTH_CASES = [
+    ("config0 single triplet L=50", [W.FE_6302], True, W.grid(W.FE_6302["lambda0"], 50, 0.024), 1000 + 7),
+    ("config1 two triplets L=128", [W.FE_6301, W.FE_6302], True, W.grid(6302.0, 128, 0.024), 2048 + 5),
+    ("full Zeeman patterns L=127 (ragged)", [W.FE_6301, W.FE_6302], False, W.grid(6302.0, 127, 0.024), 517),
+    ("single anomalous line L=3", [W.FE_6301], False, W.grid(W.FE_6301["lambda0"], 3, 0.05), 33),
+    ("config4-like grid L=256", [W.FE_6301, W.FE_6302], True, W.grid(6302.0, 256, 0.012), 300),
+    ("three lines (run-time line count) L=64", [W.FE_6301, W.FE_6302, dict(W.FE_6302, lambda0=6302.0)], True, W.grid(6302.0, 64, 0.03), 100),
+]
+
+
+@pytest.mark.parametrize("name,lines,triplets,lam,P", SYNTH_CASES, ids=[c[0] for c in SYNTH_CASES])
+def test_me_synth_vs_oracle(B, name, lines, triplets, lam, P):
+    p = W.draw_truth(P, seed=101)
+    mu = np.random.default_rng(1).uniform(0.05, 1.0, P)
+    ref = orc.synth(p, lam, oracle_lines(lines, triplets), mu=mu, threads=NTHREADS)
+    ld = B.line_data_from_workload(lines, triplets)
+    out, _ = B.me_synth(dev(p), lam, ld, mu=dev(mu))
+    out = out.cpu().numpy().astype(np.float64)
+    cont = (p[:, 7] + mu * p[:, 8])[:, None, None]
+    err = np.abs(out - ref) / cont
+    assert err.max() <= 2e-5, (name, err.max(), np.unravel_index(err.argmax(), err.shape))
+    # mu = NULL means mu = 1
+    out1, _ = B.me_synth(dev(p[:64]), lam, ld)
+    ref1 = orc.synth(p[:64], lam, oracle_lines(lines, triplets), threads=NTHREADS)
+    assert np.max(np.abs(out1.cpu().numpy() - ref1) / (p[:64, 7] + p[:64, 8])[:, None, None]) <= 2e-5
+
+
+def test_me_synth_extremes_and_chi2(B):
+    c1 = W.config1()
+    lam = c1["lam"]
+    lo, hi, _, _ = W.prior_box(1.0, 3500.0)
+    rng = np.random.default_rng(3)
+    corners = np.where(rng.random((512, 9)) < 0.5, lo, hi)        # corners of the search box
+    corners[:, 0] = np.where(rng.random(512) < 0.3, 0.0, corners[:, 0])   # and B = 0
+    ref = orc.synth(corners, lam, oracle_lines(c1["lines"], True), threads=NTHREADS)
+    ld = B.line_data_from_workload(c1["lines"], True)
+    out, _ = B.me_synth(dev(corners), lam, ld)
+    err = np.abs(out.cpu().numpy() - ref) / (corners[:, 7] + corners[:, 8])[:, None, None]
+    assert err.max() <= 2e-5
+    zero_b = corners[:, 0] == 0.0
+    assert float(out[torch.from_numpy(zero_b).cuda()][:, 1:].abs().max()) == 0.0     # B = 0 => Q = U = V = 0 exactly
+    # fused chi2 against a fixed profile (config 2), with and without the Stokes output
+    p = W.draw_truth(3000, seed=7)
+    obs = orc.synth(p[:1], lam, oracle_lines(c1["lines"], True))[0] + W.draw_noise((4, 128), 1e-3)
+    model = orc.synth(p, lam, oracle_lines(c1["lines"], True), threads=NTHREADS)
+    w, sig = c1["ga"]["stokes_weight"], c1["ga"]["sigma"]
+    want = np.array([orc.chi2(obs, m, w, sig) for m in model])
+    _, chi_a = B.me_synth(dev(p), lam, ld, obs_ref=dev(obs), w_over_sigma=w / sig)
+    _, chi_b = B.me_synth(dev(p), lam, ld, obs_ref=dev(obs), w_over_sigma=w / sig, want_stokes=False)
+    assert torch.equal(chi_a, chi_b)
+    got = chi_a.cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(got - want) / want) < 2e-4
+    assert B.me_synth(dev(p[:0]), lam, ld)[0].shape[0] == 0       # empty input
+
+
+# ---------------------------------------------------------------------------------------------------- GA stages
+@pytest.mark.parametrize("pop,k", [(64, 3), (100, 2), (128, 3), (512, 4), (2, 1), (1024, 3)])
+def test_ga_init_and_step_bit_exact(B, pop, k):
+    G = 20
+    cfg = W.ga_config(pop, G, tournament_k=k)
+    N, seed, base = 37, 0xABCDEF0123, 4000000000
+    g0 = B.ga_init(N, cfg, seed, pixel_id_base=base)
+    assert np.array_equal(g0.cpu().numpy(), orc.ga_init(N, pop, seed, pixel_base=base))
+    rng = np.random.default_rng(pop)
+    genes = rng.random((N, pop, 9)).astype(np.float32)
+    chi2 = (rng.random((N, pop)) * 50).astype(np.float32)
+    chi2[0, : pop // 2] = chi2[0, 0]                              # ties
+    chi2[1, 1] = np.inf
+    chi2[2, :] = 7.0
+    for t in (1, 7, G):
+        got = B.ga_step(dev(genes), dev(chi2), t, cfg, seed, pixel_id_base=base).cpu().numpy()
+        want = orc.ga_step(genes, chi2.astype(np.float64), t, cfg, seed, pixel_base=base)
+        assert np.array_equal(got, want), (pop, k, t)
+    # NaN fitness is treated as +Inf (reading G4)
+    chi2n = chi2.copy(); chi2n[3, 0] = np.nan
+    chi2i = chi2.copy(); chi2i[3, 0] = np.inf
+    assert torch.equal(B.ga_step(dev(genes), dev(chi2n), 2, cfg, seed), B.ga_step(dev(genes), dev(chi2i), 2, cfg, seed))
+
+
+@pytest.mark.parametrize("which", ["config0", "config1", "full_pattern"])
+def test_fused_fitness_vs_oracle(B, which):
+    cfgw = W.config0() if which == "config0" else W.config1()
+    triplets = which != "full_pattern"
+    cfgw = dict(cfgw, triplets=triplets)
+    N, pop = 24, cfgw["ga"]["pop"]
+    mu = np.linspace(0.1, 1.0, N)
+    truth, obs, ln = make_obs(cfgw, N, mu=mu, threads=NTHREADS)
+    genes = orc.ga_init(N, pop, seed=11)
+    genes[:, 0, :] = 0.0; genes[:, 1, :] = 1.0                      # box corners
+    want = orc.ga_fitness(genes, obs, cfgw["lam"], ln, cfgw["ga"], mu=mu, threads=NTHREADS)
+    ld = B.line_data_from_workload(cfgw["lines"], triplets)
+    got = B.ga_fitness(dev(genes), dev(obs), cfgw["lam"], ld, cfgw["ga"], mu=dev(mu)).cpu().numpy().astype(np.float64)
+    rel = np.abs(got - want) / want
+    assert rel.max() < 2e-4, rel.max()
+    assert np.median(rel) < 1e-5
