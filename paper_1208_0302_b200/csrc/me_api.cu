@@ -129,12 +129,12 @@ int me_synth(const float* params, int64_t P, const float* mu, const double* lamb
              const me_line_data* line_data, float* out_stokes,
              const float* obs_ref, const float* w_over_sigma, float* out_chi2, void* stream) {
     if (P < 0) return ME_ERR_SHAPE;
-    if (out_stokes == nullptr && out_chi2 == nullptr) return ME_ERR_NULL;
-    if (out_chi2 != nullptr && (obs_ref == nullptr || w_over_sigma == nullptr)) return ME_ERR_NULL;
     me::SynthDesc sd;
     int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
     if (rc != ME_OK) return rc;
     if (P == 0) return ME_OK;
+    if (out_stokes == nullptr && out_chi2 == nullptr) return ME_ERR_NULL;
+    if (out_chi2 != nullptr && (obs_ref == nullptr || w_over_sigma == nullptr)) return ME_ERR_NULL;
     if (params == nullptr) return ME_ERR_NULL;
     float w2[4] = {0, 0, 0, 0};
     if (out_chi2 != nullptr)
