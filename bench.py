@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py — whole-hot-path throughput of the GA inversion (ga_invert) on synthetic SOLIS/VSM-shaped maps.
+
+A "step" is one pass of the whole hot path over one batch: one `ga_invert` call (observation staging, generation 0,
+G generations of select/crossover/mutate/evaluate, output) over the map of the chosen workload.
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config1|config3|config0] [--impl reference]
+One JSON line on stdout (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1208_0302_b200 import workloads as W  # noqa: E402
+
+# FP32 work per wavelength point of the fused fitness loop, counted from an ncu capture of this workload
+# (profiles/: smsp__sass_thread_inst_executed_op_{ffma,fmul,fadd}_pred_on / lambda-points; FFMA = 2 flop).
+# See DESIGN.md "Roofline".  Keyed by workload name.
+FLOP_PER_POINT = {"config0_tiny": 260.0, "config1_map256": 477.0, "config3_fulldisc": 477.0}
+SM_COUNT, FP32_LANES_PER_SM = 148, 128
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config3"])
+    ap.add_argument("--n-side", type=int, default=0, help="override the map side (config1: 256, config3: 2048)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload(args):
+    if args.workload == "config0":
+        c = W.config0()
+        return c, c["n_pixels"], None
+    if args.workload == "config1":
+        side = args.n_side or 256
+        c = W.config1(side)
+        return c, side * side, None
+    side = args.n_side or 2048
+    c = W.config3(side)
+    return c, side * side, side
+
+
+def syntheses_per_pixel(ga):
+    return ga["pop"] + ga["generations"] * (ga["pop"] - 1)
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
+
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc is not None:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.thr.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "power_w_max": float(max(pw)), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+def oracle_lines_for(cfg):
+    from oracle import api as orc
+    lines = [dict(lambda0=l["lambda0"], strength=l["strength"], shift=[0.0, -l["g_eff"], l["g_eff"]], weight=[1, 1, 1],
+                  kind=[0, -1, 1]) for l in cfg["lines"]]
+    return orc.Lines(lines, W.LAMBDA_REF)
+
+
+def oracle_sample(cfg, n, stream=0):
+    """n pixels of the workload, observations synthesised by the oracle itself (+ seeded noise, rounded to f32)."""
+    from oracle import api as orc
+    ln = oracle_lines_for(cfg)
+    truth = W.draw_truth(n, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=100 + stream)
+    clean = orc.synth(truth, cfg["lam"], ln, threads=orc.hardware_threads())
+    obs = (clean + W.draw_noise(clean.shape, cfg["sigma"], stream=100 + stream)).astype(np.float32).astype(np.float64)
+    return ln, obs
+
+
+def time_oracle(cfg, n, stream=0):
+    from oracle import api as orc
+    ln, obs = oracle_sample(cfg, n, stream)
+    cores = orc.hardware_threads()
+    t0 = time.perf_counter()
+    orc.ga_invert(obs, cfg["lam"], ln, cfg["ga"], seed=W.SEED_GA, threads=cores)
+    return time.perf_counter() - t0, cores
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import api as orc
+    cfg, n_pixels, _ = workload(args)
+    cores = orc.hardware_threads()
+    per_pixel_points = syntheses_per_pixel(cfg["ga"]) * cfg["lam"].size * sum(3 for _ in cfg["lines"])
+    n = max(cores, int(cores * max(1.0, 2.0e7 / per_pixel_points)))      # ~ a few seconds of work per core per step
+    n = min(n, n_pixels)
+    for w in range(args.warmup):
+        time_oracle(cfg, n, stream=w)
+    t = 0.0
+    for k in range(args.steps):
+        dt, _ = time_oracle(cfg, n, stream=args.warmup + k)
+        t += dt
+    val = n * args.steps / t
+    sample = "%d pixels of %s per step (oracle-synthesised obs), all %d host threads" % (n, cfg["name"], cores)
+    line = {"impl": "reference", "metric": "pixel-inversions/s", "value": val, "unit": "pixels/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "pixels_per_step": n, "L": int(cfg["lam"].size), "pop": cfg["ga"]["pop"],
+                       "generations": cfg["ga"]["generations"], "lines": len(cfg["lines"])},
+            "syntheses_per_s": val * syntheses_per_pixel(cfg["ga"]),
+            "cpu_baseline": {"value": val, "unit": "pixels/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "pixels/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ GPU leg
+def build_inputs(cfg, n_pixels, side, rank, torch, B):
+    """Synthetic observation cube resident in HBM: truth -> me_synth (this library) -> + Gaussian noise (device RNG)."""
+    dev = torch.device("cuda")
+    if side is None:
+        truth = W.draw_truth(n_pixels, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=rank)
+        mask_t = mu_t = None
+        n_active = n_pixels
+    else:
+        mask, mu, truth, _ = W.fulldisc_truth(cfg["n_side"], cfg["radius"], seed=W.SEED_TRUTH + rank)
+        mask_t = torch.from_numpy(mask).to(dev)
+        mu_t = torch.from_numpy(mu.astype(np.float32)).to(dev)
+        n_active = int(mask.sum())
+    ld = B.line_data_from_workload(cfg["lines"], cfg["triplets"])
+    truth_t = torch.from_numpy(truth.astype(np.float32)).to(dev)
+    obs, _ = B.me_synth(truth_t, cfg["lam"], ld, mu=mu_t)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(W.SEED_NOISE + 1000 * rank)
+    chunk = 1 << 18
+    for s in range(0, n_pixels, chunk):                       # in place, bounded temporaries
+        o = obs[s:s + chunk]
+        o.add_(torch.randn(o.shape, generator=gen, device=dev, dtype=torch.float32), alpha=float(cfg["sigma"]))
+    torch.cuda.synchronize()
+    return ld, obs, mask_t, mu_t, n_active, truth
+
+
+def run_b200(args):
+    import torch
+    from paper_1208_0302_b200 import binding as B, build as mebuild
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if rank == 0:
+        mebuild.build()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    B.lib()
+    cfg, n_pixels, side = workload(args)
+    ld, obs, mask_t, mu_t, n_active, _ = build_inputs(cfg, n_pixels, side, rank, torch, B)
+    ga, lam = cfg["ga"], cfg["lam"]
+    base = rank * n_pixels                                    # shards keyed by global pixel id (no data-path collective)
+    out_p = torch.empty((n_pixels, 9), dtype=torch.float32, device="cuda")
+    out_c = torch.empty((n_pixels,), dtype=torch.float32, device="cuda")
+
+    def step():
+        B.ga_invert(obs, lam, ld, ga, W.SEED_GA, mask=mask_t, mu=mu_t, pixel_id_base=base, out_params=out_p, out_chi2=out_c)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+        ev1.record()
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
+    med_chi2 = float(out_c[~torch.isnan(out_c)].median().item())
+
+    # end to end through the C ABI from HOST buffers: pinned obs -> H2D -> ga_invert -> D2H of params + chi2
+    e2e = None
+    if not args.no_e2e:
+        h_obs = torch.empty(obs.shape, dtype=torch.float32, pin_memory=True); h_obs.copy_(obs)
+        h_p = torch.empty(out_p.shape, dtype=torch.float32, pin_memory=True)
+        h_c = torch.empty(out_c.shape, dtype=torch.float32, pin_memory=True)
+        d_obs = torch.empty_like(obs)
+        h2d = h_obs.numel() * 4
+        d2h = (h_p.numel() + h_c.numel()) * 4
+
+        def e2e_step():
+            d_obs.copy_(h_obs, non_blocking=True)
+            B.ga_invert(d_obs, lam, ld, ga, W.SEED_GA, mask=mask_t, mu=mu_t, pixel_id_base=base, out_params=out_p, out_chi2=out_c)
+            h_p.copy_(out_p, non_blocking=True); h_c.copy_(out_c, non_blocking=True)
+
+        e2e_step(); barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_e2e = max(1, min(args.steps, 2))
+        e0.record()
+        for _ in range(n_e2e):
+            e2e_step()
+        e1.record(); barrier()
+        ems = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ems], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ems = float(t.item())
+        e2e = {"value": world * n_active * n_e2e / (ems * 1e-3), "unit": "pixels/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": n_e2e}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    sec = ms * 1e-3
+    value = world * n_active * args.steps / sec
+    syn = syntheses_per_pixel(ga)
+    L = int(lam.size)
+    points_per_launch = n_active * syn * L
+    flop_pt = FLOP_PER_POINT[cfg["name"]]
+    launch_s = sec / args.steps
+    achieved = flop_pt * points_per_launch / launch_s / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    clocks = clk.summary()
+    line = {"metric": "pixel-inversions/s", "value": value, "unit": "pixels/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["name"], "pixels_per_gpu": n_pixels, "active_pixels_per_gpu": n_active, "L": L,
+                       "pop": ga["pop"], "generations": ga["generations"], "lines": len(cfg["lines"]),
+                       "zeeman": "effective triplets", "parallelism": "pixel shards x%d" % world,
+                       "l2": "obs cube %.0f MB per step (> 126 MB L2 for config1/3); path is ALU-bound" % (obs.numel() * 4 / 1e6)},
+            "syntheses_per_s": value * syn, "median_chi2": med_chi2,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt,
+                         "peak_basis": "148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (max SM clock)" % sm_max,
+                         "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / sm_max)) if clocks.get("sm_mhz") else None},
+            "clocks": clocks, "gpu_launches": args.steps, "e2e": e2e}
+    if not args.no_cpu_baseline:
+        from oracle import api as orc
+        cores = orc.hardware_threads()
+        n = min(n_pixels, 2 * cores)
+        dt, cores = time_oracle(cfg, n)
+        line["cpu_baseline"] = {"value": n / dt, "unit": "pixels/s", "cores": cores, "kind": "oracle",
+                                "sample": "%d pixels of %s, oracle-synthesised obs, %.1f s" % (n, cfg["name"], dt)}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_b200(a)
