@@ -1,8 +1,8 @@
 // me_device.cuh — device-side building blocks of libme_b200.so (sm_100a, FP32).
 //
-//   faddeeva32      w(v + i a) = H + iF, two-region FP32 evaluator
+//   faddeeva_pair   w(v + i a) = H + iF on two wavelengths, two-region FP32 evaluator
 //   Individual      per-parameter-vector constants hoisted out of the wavelength loop (eq. 14)
-//   stokes_at       absorption matrix (eq. 8) + Unno-Rachkovsky solution (eq. 12-13, 15) at one wavelength
+//   stokes_pair     absorption matrix (eq. 8) + Unno-Rachkovsky solution (eq. 12-13, 15) at two wavelengths
 //   philox4x32_10   counter-based RNG keyed by (seed; pixel, generation, individual, block)
 //   make_child      tournament selection, arithmetic crossover, bounded mutation
 //
@@ -31,7 +31,7 @@ struct LineDesc {
     int pad[2];
 };
 
-struct SynthDesc {
+struct alignas(16) SynthDesc {
     int L, n_lines, n_comp, all_triplets;
     LineDesc line[ME_MAX_LINES];
     float shift[ME_MAX_COMP];
@@ -52,74 +52,98 @@ struct GaDesc {
 };
 
 // ------------------------------------------------------------------------------------------------------------
-// Small helpers
+// Packed FP32 helpers.  Blackwell (sm_100) issues two FP32 FMAs per instruction (FFMA2 / FMUL2 / FADD2); the FMA
+// pipe is as wide as before, so packing halves the ISSUE slots of the arithmetic.  The fitness loop is issue-bound
+// (profiles/r1a), so everything per wavelength is written on pairs of adjacent wavelengths (j, j+1) held in float2.
+// Scalars broadcast for free (SASS operand form R.F32), negation is an operand modifier.
 // ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ float rcp_approx(float x) {
+typedef float2 f2;
+#define MEDEV __device__ __forceinline__
+
+MEDEV f2 bc(float s) { return make_float2(s, s); }
+MEDEV f2 neg(f2 a) { return make_float2(-a.x, -a.y); }
+MEDEV f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+MEDEV f2 fma2(float a, f2 b, f2 c) { return __ffma2_rn(bc(a), b, c); }
+MEDEV f2 fma2(f2 a, f2 b, float c) { return __ffma2_rn(a, b, bc(c)); }
+MEDEV f2 fma2(float a, f2 b, float c) { return __ffma2_rn(bc(a), b, bc(c)); }
+MEDEV f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+MEDEV f2 mul2(float a, f2 b) { return __fmul2_rn(bc(a), b); }
+MEDEV f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+MEDEV f2 sub2(f2 a, f2 b) { return __fadd2_rn(a, neg(b)); }
+
+MEDEV float rcp_approx(float x) {
     float y;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+MEDEV f2 rcp2(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
 
-// p <- p * Z + c   (complex p, complex Z, real c): 4 FP32 instructions
-__device__ __forceinline__ void chorner(float& pr, float& pi, float zr, float zi, float c) {
-    float nr = fmaf(pr, zr, c);
-    nr = fmaf(-pi, zi, nr);
-    float ni = pr * zi;
-    ni = fmaf(pi, zr, ni);
-    pr = nr; pi = ni;
-}
+// Real-coefficient polynomial at a complex argument x by the quadratic-factor recurrence
+//   b_k = c_k + t b_{k+1} + m b_{k+2},  t = 2 Re x,  m = -|x|^2;   P(x) = (b_0 - b_1 Re x) + i b_1 Im x
+// (x^2 = t x + m): two FMAs per coefficient instead of four for a complex Horner step.
+#define ME_REC(bk, ck, b1, b2) const f2 bk = fma2(t, b1, fma2(m, b2, ck))
 
 // ------------------------------------------------------------------------------------------------------------
-// Faddeeva function, FP32.  a2 = a*a and La = L + a, La2 = La*La are per-individual constants.
-//   wing: w = (i/sqrt(pi)) s R(q), s = 1/z, q = s^2 (no cancellation: H keeps full relative accuracy)
-//   core: Weideman N = 16
+// Faddeeva function w(v + i a) = H + iF on a pair of v, FP32, two regions.
+//   wing |z|^2 >= CUT2: w = (i/sqrt(pi)) s R(q), s = 1/z, q = s^2, R = asymptotic series to q^6.  H comes out as
+//                       a/(sqrt(pi)|z|^2) x (1 + ...): no cancellation, full relative accuracy.
+//   core |z|^2 <  CUT2: Weideman (1994), N = FAD_N terms in Z = (L + iz)/(L - iz).
 // ------------------------------------------------------------------------------------------------------------
-struct FadConst { float a, a2, La, La2; };
+struct FadConst { float a, a2, two_a, La, La2, Lma2; };
 
-__device__ __forceinline__ FadConst fad_const(float a) {
-    FadConst f; f.a = a; f.a2 = a * a; f.La = FAD_L + a; f.La2 = f.La * f.La; return f;
+MEDEV FadConst fad_const(float a) {
+    FadConst f;
+    f.a = a; f.a2 = a * a; f.two_a = 2.0f * a;
+    f.La = FAD_L + a; f.La2 = f.La * f.La;
+    f.Lma2 = (FAD_L - a) * (FAD_L - a);
+    return f;
 }
 
-__device__ __forceinline__ void faddeeva32(float v, const FadConst& f, float& wr, float& wi) {
-    const float r2 = fmaf(v, v, f.a2);
-    if (r2 >= FAD_CUT2) {
-        const float r = rcp_approx(r2);
-        const float sr = v * r, si = -f.a * r;
-        const float qr = fmaf(sr, sr, -si * si), qi = 2.0f * sr * si;
-        float pr = fmaf(FAD_C6, qr, FAD_C5), pi = FAD_C6 * qi;
-        chorner(pr, pi, qr, qi, FAD_C4);
-        chorner(pr, pi, qr, qi, FAD_C3);
-        chorner(pr, pi, qr, qi, FAD_C2);
-        chorner(pr, pi, qr, qi, FAD_C1);
-        chorner(pr, pi, qr, qi, FAD_C0);
-        wr = -fmaf(sr, pi, si * pr);
-        wi = fmaf(sr, pr, -si * pi);
-    } else {
-        const float r = rcp_approx(fmaf(v, v, f.La2));
-        const float dr = f.La * r, di = v * r;                 // D = 1 / (L - iz)
-        const float zr = fmaf(FAD_2L, dr, -1.0f), zi = FAD_2L * di;   // Z = (L + iz) D = 2 L D - 1
-        float pr = fmaf(FAD_A15, zr, FAD_A14), pi = FAD_A15 * zi;
-        chorner(pr, pi, zr, zi, FAD_A13);
-        chorner(pr, pi, zr, zi, FAD_A12);
-        chorner(pr, pi, zr, zi, FAD_A11);
-        chorner(pr, pi, zr, zi, FAD_A10);
-        chorner(pr, pi, zr, zi, FAD_A9);
-        chorner(pr, pi, zr, zi, FAD_A8);
-        chorner(pr, pi, zr, zi, FAD_A7);
-        chorner(pr, pi, zr, zi, FAD_A6);
-        chorner(pr, pi, zr, zi, FAD_A5);
-        chorner(pr, pi, zr, zi, FAD_A4);
-        chorner(pr, pi, zr, zi, FAD_A3);
-        chorner(pr, pi, zr, zi, FAD_A2);
-        chorner(pr, pi, zr, zi, FAD_A1);
-        chorner(pr, pi, zr, zi, FAD_A0);
-        // w = D (p D + 1/sqrt(pi))   (the factor 2 is folded into the table)
-        float tr = fmaf(pr, dr, FAD_INV_SQRTPI);
-        tr = fmaf(-pi, di, tr);
-        float ti = pr * di;
-        ti = fmaf(pi, dr, ti);
-        wr = fmaf(dr, tr, -di * ti);
-        wi = fmaf(dr, ti, di * tr);
+MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
+    const f2 r = rcp2(r2);                                    // 1/|z|^2
+    const f2 rr = mul2(r, r);                                 // 1/|z|^4 = |q|^2
+    const f2 m = neg(rr);                                     // -|q|^2
+    const f2 qr = mul2(fma2(v, v, -f.a2), rr);                // Re q = (v^2 - a^2)/|z|^4
+    const f2 nqi = mul2(mul2(f.two_a, v), rr);                // -Im q = 2 v a/|z|^4
+    const f2 t = add2(qr, qr);
+    const f2 b5 = fma2(t, bc(FAD_C6), FAD_C5);
+    const f2 b4 = fma2(t, b5, fma2(m, bc(FAD_C6), FAD_C4));
+    ME_REC(b3, FAD_C3, b4, b5);
+    ME_REC(b2, FAD_C2, b3, b4);
+    ME_REC(b1, FAD_C1, b2, b3);
+    ME_REC(b0, FAD_C0, b1, b2);
+    const f2 Rr = fma2(neg(b1), qr, b0);                      // Re R
+    const f2 nRi = mul2(b1, nqi);                             // -Im R
+    // w = i s R = r (a + i v)(Rr + i Ri)
+    wr = mul2(r, fma2(f.a, Rr, mul2(v, nRi)));
+    wi = mul2(r, fma2(v, Rr, mul2(-f.a, nRi)));
+}
+
+MEDEV void faddeeva_core(f2 v, const FadConst& f, f2& wr, f2& wi) {
+    const f2 v2 = mul2(v, v);
+    const f2 r = rcp2(add2(v2, bc(f.La2)));                   // 1/|L - iz|^2
+    const f2 dr = mul2(f.La, r), di = mul2(v, r);             // D = 1/(L - iz)
+    const f2 zr = fma2(FAD_2L, dr, -1.0f), zi = mul2(FAD_2L, di);   // Z = (L + iz) D = 2 L D - 1
+    const f2 t = add2(zr, zr);
+    const f2 m = neg(mul2(add2(v2, bc(f.Lma2)), r));          // -|Z|^2 = -|L + iz|^2 / |L - iz|^2
+    FAD_CORE_RECURRENCE(t, m)
+    const f2 Pr = fma2(neg(cb1), zr, cb0), Pi = mul2(cb1, zi);   // p(Z), the factor 2 folded into the table
+    // w = D (p D + 1/sqrt(pi))
+    const f2 tr = fma2(neg(Pi), di, fma2(Pr, dr, FAD_INV_SQRTPI));
+    const f2 ti = fma2(Pi, dr, mul2(Pr, di));
+    wr = fma2(dr, tr, neg(mul2(di, ti)));
+    wi = fma2(dr, ti, mul2(di, tr));
+}
+
+MEDEV void faddeeva_pair(f2 v, const FadConst& f, f2& wr, f2& wi) {
+    const f2 r2 = fma2(v, v, f.a2);
+    const bool w0 = r2.x >= FAD_CUT2, w1 = r2.y >= FAD_CUT2;
+    if (w0 || w1) faddeeva_wing(v, r2, f, wr, wi);
+    if (!(w0 && w1)) {
+        f2 cr, ci;
+        faddeeva_core(v, f, cr, ci);
+        if (!w0) { wr.x = cr.x; wi.x = ci.x; }
+        if (!w1) { wr.y = cr.y; wi.y = ci.y; }
     }
 }
 
@@ -136,7 +160,7 @@ struct Individual {
 };
 
 template <int NL>
-__device__ __forceinline__ void setup_individual(Individual<NL>& ind, const float* p, float mu, const SynthDesc& d) {
+MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const SynthDesc& d) {
     const float B = p[0], eta0 = p[3], dld = p[4], a = p[5], vlos = p[6];
     float sg, cg;
     sincospif(p[1] * (1.0f / 180.0f), &sg, &cg);
@@ -158,67 +182,69 @@ __device__ __forceinline__ void setup_individual(Individual<NL>& ind, const floa
     }
 }
 
-// Profile sums of one line at reduced wavelength v:  S_kind += r_l * sum_c weight_c * w(v - shift_c vB + i a)
+// Profile sums of one line at a pair of reduced wavelengths v:
+//   S_kind += r_l * sum_c weight_c * w(v - shift_c vB + i a)
 template <bool TRIPLET>
-__device__ __forceinline__ void line_profiles(float v, float vB, const FadConst& fad, const SynthDesc& d, int l,
-                                              float& br, float& bi, float& pr, float& pi, float& rr, float& ri) {
+MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const SynthDesc& d, int l,
+                         f2& br, f2& bi, f2& pr, f2& pi, f2& rr, f2& ri) {
     const float r = d.line[l].strength;
     if (TRIPLET) {
         const float gvB = d.line[l].g * vB;
-        float w0r, w0i, w1r, w1i, w2r, w2i;
-        faddeeva32(v, fad, w0r, w0i);
-        faddeeva32(v + gvB, fad, w1r, w1i);      // sigma_blue sits at v = -g vB
-        faddeeva32(v - gvB, fad, w2r, w2i);      // sigma_red  sits at v = +g vB
-        pr = fmaf(r, w0r, pr); pi = fmaf(r, w0i, pi);
-        br = fmaf(r, w1r, br); bi = fmaf(r, w1i, bi);
-        rr = fmaf(r, w2r, rr); ri = fmaf(r, w2i, ri);
+        f2 w0r, w0i, w1r, w1i, w2r, w2i;
+        faddeeva_pair(v, fad, w0r, w0i);
+        faddeeva_pair(add2(v, bc(gvB)), fad, w1r, w1i);      // sigma_blue sits at v = -g vB
+        faddeeva_pair(add2(v, bc(-gvB)), fad, w2r, w2i);     // sigma_red  sits at v = +g vB
+        pr = fma2(r, w0r, pr); pi = fma2(r, w0i, pi);
+        br = fma2(r, w1r, br); bi = fma2(r, w1i, bi);
+        rr = fma2(r, w2r, rr); ri = fma2(r, w2i, ri);
     } else {
         const int* kb = d.line[l].kind_begin;
         for (int c = kb[0]; c < kb[1]; ++c) {
-            float wr, wi; faddeeva32(fmaf(-d.shift[c], vB, v), fad, wr, wi);
-            const float s = r * d.weight[c]; br = fmaf(s, wr, br); bi = fmaf(s, wi, bi);
+            f2 wr, wi; faddeeva_pair(add2(v, bc(-d.shift[c] * vB)), fad, wr, wi);
+            const float s = r * d.weight[c]; br = fma2(s, wr, br); bi = fma2(s, wi, bi);
         }
         for (int c = kb[1]; c < kb[2]; ++c) {
-            float wr, wi; faddeeva32(fmaf(-d.shift[c], vB, v), fad, wr, wi);
-            const float s = r * d.weight[c]; pr = fmaf(s, wr, pr); pi = fmaf(s, wi, pi);
+            f2 wr, wi; faddeeva_pair(add2(v, bc(-d.shift[c] * vB)), fad, wr, wi);
+            const float s = r * d.weight[c]; pr = fma2(s, wr, pr); pi = fma2(s, wi, pi);
         }
         for (int c = kb[2]; c < kb[3]; ++c) {
-            float wr, wi; faddeeva32(fmaf(-d.shift[c], vB, v), fad, wr, wi);
-            const float s = r * d.weight[c]; rr = fmaf(s, wr, rr); ri = fmaf(s, wi, ri);
+            f2 wr, wi; faddeeva_pair(add2(v, bc(-d.shift[c] * vB)), fad, wr, wi);
+            const float s = r * d.weight[c]; rr = fma2(s, wr, rr); ri = fma2(s, wi, ri);
         }
     }
 }
 
-// Stokes vector at wavelength index j (eq. 8 + eq. 12-13 times I_c of eq. 15).
+// Stokes vectors at the wavelength pair (j0, j1) (eq. 8 + eq. 12-13 times I_c of eq. 15).  j1 = j0 + 1 with j0 even
+// in the main loop (one 8-byte constant-bank load per line); j1 = j0 for the odd tail.
 // The Unno-Rachkovsky solution is evaluated in the frame chi = 0 (eta_U = rho_U = 0) and Q,U are rotated by 2 chi.
 template <int NL, bool TRIPLET>
-__device__ __forceinline__ void stokes_at(const Individual<NL>& ind, const SynthDesc& d, int j,
-                                          float& I, float& Q, float& U, float& V) {
-    float br = 0.f, bi = 0.f, pr = 0.f, pi = 0.f, rr = 0.f, ri = 0.f;
+MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2& I, f2& Q, f2& U, f2& V) {
+    f2 br = bc(0.f), bi = bc(0.f), pr = bc(0.f), pi = bc(0.f), rr = bc(0.f), ri = bc(0.f);
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
         if (NL == ME_MAX_LINES && l >= d.n_lines) break;      // NL == ME_MAX_LINES is the run-time-sized fallback
-        const float v = fmaf(d.off[l][j], ind.invD[l], ind.v0[l]);
+        const f2 off = tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]);
+        const f2 v = fma2(ind.invD[l], off, ind.v0[l]);
         line_profiles<TRIPLET>(v, ind.vB[l], ind.fad, d, l, br, bi, pr, pi, rr, ri);
     }
-    const float sr = br + rr, si = bi + ri;                       // sigma sum
-    const float eI = fmaf(ind.kA, pr, fmaf(ind.kB, sr, 1.0f));
-    const float eL = ind.kA * fmaf(-0.5f, sr, pr);                // eta_Q in the chi = 0 frame
-    const float rL = ind.kA * fmaf(-0.5f, si, pi);                // rho_Q in the chi = 0 frame
-    const float eV = ind.kC * (rr - br);
-    const float rV = ind.kC * (ri - bi);
-    const float eI2 = eI * eI;
-    const float Pi = fmaf(eL, rL, eV * rV);
-    const float rho2 = fmaf(rL, rL, rV * rV);
-    const float eta2 = fmaf(eL, eL, eV * eV);
-    const float Delta = fmaf(eI2, eI2 + (rho2 - eta2), -Pi * Pi);
-    const float t = ind.muS1 * rcp_approx(Delta);
-    I = fmaf(t * eI, eI2 + rho2, ind.S0);
-    const float Qp = -t * fmaf(eI2, eL, rL * Pi);
-    const float Up = -t * eI * fmaf(eL, rV, -eV * rL);
-    V = -t * fmaf(eI2, eV, rV * Pi);
-    Q = fmaf(Qp, ind.c2x, -Up * ind.s2x);
-    U = fmaf(Qp, ind.s2x, Up * ind.c2x);
+    const f2 sr = add2(br, rr), si = add2(bi, ri);                // sigma sums
+    const f2 eI = fma2(ind.kA, pr, fma2(ind.kB, sr, 1.0f));
+    const f2 eL = mul2(ind.kA, fma2(-0.5f, sr, pr));              // eta_Q in the chi = 0 frame
+    const f2 rL = mul2(ind.kA, fma2(-0.5f, si, pi));              // rho_Q in the chi = 0 frame
+    const f2 eV = mul2(ind.kC, sub2(rr, br));
+    const f2 rV = mul2(ind.kC, sub2(ri, bi));
+    const f2 eI2 = mul2(eI, eI);
+    const f2 Pi = fma2(eL, rL, mul2(eV, rV));
+    const f2 rho2 = fma2(rL, rL, mul2(rV, rV));
+    const f2 eta2 = fma2(eL, eL, mul2(eV, eV));
+    const f2 Delta = fma2(eI2, add2(eI2, sub2(rho2, eta2)), neg(mul2(Pi, Pi)));
+    const f2 nt = mul2(-ind.muS1, rcp2(Delta));                   // -mu S1 / Delta
+    I = fma2(mul2(neg(nt), eI), add2(eI2, rho2), ind.S0);
+    const f2 Qp = mul2(nt, fma2(eI2, eL, mul2(rL, Pi)));
+    const f2 Up = mul2(mul2(nt, eI), fma2(eL, rV, neg(mul2(eV, rL))));
+    V = mul2(nt, fma2(eI2, eV, mul2(rV, Pi)));
+    Q = fma2(ind.c2x, Qp, mul2(-ind.s2x, Up));
+    U = fma2(ind.s2x, Qp, mul2(ind.c2x, Up));
 }
 
 // ------------------------------------------------------------------------------------------------------------

@@ -16,7 +16,7 @@ namespace me {
 
 // ------------------------------------------------------------------------------------------------------------
 // Fitness of one individual held in registers: decode -> per-individual constants -> wavelength loop.
-// obs_s: shared memory, [L] float4 = (I,Q,U,V) at each wavelength (broadcast reads, conflict-free).
+// obs_s: shared memory, per wavelength pair two float4 = (I0,I1,Q0,Q1), (U0,U1,V0,V1) (broadcast reads, conflict-free).
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET>
 __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
@@ -26,25 +26,35 @@ __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDe
     for (int j = 0; j < ME_NPAR; ++j) p[j] = decode_gene(g[j], gd, j);
     Individual<NL> ind;
     setup_individual<NL>(ind, p, mu, sd);
-    float aI = 0.f, aQ = 0.f, aU = 0.f, aV = 0.f;
-    const int L = sd.L;
-    for (int j = 0; j < L; ++j) {
-        float I, Q, U, V;
-        stokes_at<NL, TRIPLET>(ind, sd, j, I, Q, U, V);
-        const float4 o = obs_s[j];
-        const float dI = o.x - I, dQ = o.y - Q, dU = o.z - U, dV = o.w - V;
-        aI = fmaf(dI, dI, aI); aQ = fmaf(dQ, dQ, aQ); aU = fmaf(dU, dU, aU); aV = fmaf(dV, dV, aV);
+    f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
+    const int L = sd.L, npair = L >> 1;
+    for (int jp = 0; jp < npair; ++jp) {
+        f2 I, Q, U, V;
+        stokes_pair<NL, TRIPLET>(ind, sd, 2 * jp, false, I, Q, U, V);
+        const float4 o0 = obs_s[2 * jp], o1 = obs_s[2 * jp + 1];           // (I0,I1,Q0,Q1), (U0,U1,V0,V1)
+        const f2 dI = sub2(make_float2(o0.x, o0.y), I), dQ = sub2(make_float2(o0.z, o0.w), Q);
+        const f2 dU = sub2(make_float2(o1.x, o1.y), U), dV = sub2(make_float2(o1.z, o1.w), V);
+        aI = fma2(dI, dI, aI); aQ = fma2(dQ, dQ, aQ); aU = fma2(dU, dU, aU); aV = fma2(dV, dV, aV);
     }
-    float chi2 = gd.inv_nu * fmaf(gd.w2[0], aI, fmaf(gd.w2[1], aQ, fmaf(gd.w2[2], aU, gd.w2[3] * aV)));
+    if (L & 1) {                                                            // odd tail: second half is a duplicate, dropped
+        f2 I, Q, U, V;
+        stokes_pair<NL, TRIPLET>(ind, sd, L - 1, true, I, Q, U, V);
+        const float4 o0 = obs_s[2 * npair], o1 = obs_s[2 * npair + 1];
+        const float dI = o0.x - I.x, dQ = o0.z - Q.x, dU = o1.x - U.x, dV = o1.z - V.x;
+        aI.x = fmaf(dI, dI, aI.x); aQ.x = fmaf(dQ, dQ, aQ.x); aU.x = fmaf(dU, dU, aU.x); aV.x = fmaf(dV, dV, aV.x);
+    }
+    const float sI = aI.x + aI.y, sQ = aQ.x + aQ.y, sU = aU.x + aU.y, sV = aV.x + aV.y;
+    float chi2 = gd.inv_nu * fmaf(gd.w2[0], sI, fmaf(gd.w2[1], sQ, fmaf(gd.w2[2], sU, gd.w2[3] * sV)));
     if (!(chi2 < __int_as_float(0x7f800000))) chi2 = __int_as_float(0x7f800000);   // NaN / Inf -> +Inf (reading G4)
     return chi2;
 }
 
-// Stage obs[n] ([4][L] in HBM, rows contiguous => coalesced) into shared memory as [L] float4.
+// Stage obs[n] ([4][L] in HBM, rows contiguous => coalesced) into shared memory, pair-interleaved:
+// element (s, j) -> word 8 (j/2) + 2 s + (j & 1).  Shared size: 8 * ceil(L/2) floats.
 __device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int L, int tid, int nthreads) {
     for (int k = tid; k < 4 * L; k += nthreads) {
         const int s = k / L, j = k - s * L;
-        obs_s[4 * j + s] = __ldg(obs_n + k);
+        obs_s[8 * (j >> 1) + 2 * s + (j & 1)] = __ldg(obs_n + k);
     }
 }
 
@@ -68,7 +78,7 @@ __device__ __forceinline__ void block_argmin(float v, int idx, uint32_t* scratch
 
 // ------------------------------------------------------------------------------------------------------------
 // The fused GA inversion kernel.
-// Dynamic shared memory: obs_s [L] float4 | genes [2][pop][9] | chi2 [2][pop] | scratch [64]
+// Dynamic shared memory: obs_s [ceil(L/2)] 2 x float4 | genes [2][pop][9] | chi2 [2][pop] | scratch [64]
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -78,7 +88,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
     extern __shared__ float4 smem4[];
     const int L = sd.L, pop = gd.pop;
     float* obs_s = reinterpret_cast<float*>(smem4);
-    float* genes_s = obs_s + 4 * L;
+    float* genes_s = obs_s + 8 * ((L + 1) >> 1);
     float* chi2_s = genes_s + 2 * pop * ME_NPAR;
     uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + 2 * pop);
     const int tid = threadIdx.x;
@@ -144,7 +154,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// me_synth: warp = parameter vector, lane = wavelength.  out_stokes[P,4,L]: each (vector, Stokes) row is
+// me_synth: warp = parameter vector, lane = wavelength pair.  out_stokes[P,4,L]: each (vector, Stokes) row is
 // written as consecutive 128-byte warp stores.  chi2 (optional) is reduced with warp shuffles.
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET>
@@ -165,17 +175,31 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
         setup_individual<NL>(ind, p, mu, sd);
         float acc = 0.f;
         float* o = out_stokes != nullptr ? out_stokes + v * 4 * (int64_t)L : nullptr;
-        for (int j = lane; j < L; j += 32) {
-            float I, Q, U, V;
-            stokes_at<NL, TRIPLET>(ind, sd, j, I, Q, U, V);
+        const bool even = (L & 1) == 0;                      // float2 rows are 8-byte aligned only for even L
+        for (int j = 2 * lane; j < L; j += 64) {
+            const bool tail = j + 1 >= L;
+            f2 I, Q, U, V;
+            stokes_pair<NL, TRIPLET>(ind, sd, j, tail, I, Q, U, V);
             if (o != nullptr) {
-                __stcs(o + j, I); __stcs(o + L + j, Q); __stcs(o + 2 * L + j, U); __stcs(o + 3 * L + j, V);
+                if (even) {
+                    __stcs(reinterpret_cast<float2*>(o + j), I); __stcs(reinterpret_cast<float2*>(o + L + j), Q);
+                    __stcs(reinterpret_cast<float2*>(o + 2 * L + j), U); __stcs(reinterpret_cast<float2*>(o + 3 * L + j), V);
+                } else {
+                    __stcs(o + j, I.x); __stcs(o + L + j, Q.x); __stcs(o + 2 * L + j, U.x); __stcs(o + 3 * L + j, V.x);
+                    if (!tail) { __stcs(o + j + 1, I.y); __stcs(o + L + j + 1, Q.y); __stcs(o + 2 * L + j + 1, U.y); __stcs(o + 3 * L + j + 1, V.y); }
+                }
             }
             if (out_chi2 != nullptr) {
-                const float dI = __ldg(obs_ref + j) - I, dQ = __ldg(obs_ref + L + j) - Q;
-                const float dU = __ldg(obs_ref + 2 * L + j) - U, dV = __ldg(obs_ref + 3 * L + j) - V;
+                const float dI = __ldg(obs_ref + j) - I.x, dQ = __ldg(obs_ref + L + j) - Q.x;
+                const float dU = __ldg(obs_ref + 2 * L + j) - U.x, dV = __ldg(obs_ref + 3 * L + j) - V.x;
                 acc = fmaf(w2I * dI, dI, acc); acc = fmaf(w2Q * dQ, dQ, acc);
                 acc = fmaf(w2U * dU, dU, acc); acc = fmaf(w2V * dV, dV, acc);
+                if (!tail) {
+                    const float eI = __ldg(obs_ref + j + 1) - I.y, eQ = __ldg(obs_ref + L + j + 1) - Q.y;
+                    const float eU = __ldg(obs_ref + 2 * L + j + 1) - U.y, eV = __ldg(obs_ref + 3 * L + j + 1) - V.y;
+                    acc = fmaf(w2I * eI, eI, acc); acc = fmaf(w2Q * eQ, eQ, acc);
+                    acc = fmaf(w2U * eU, eU, acc); acc = fmaf(w2V * eV, eV, acc);
+                }
             }
         }
         if (out_chi2 != nullptr) {
@@ -267,9 +291,9 @@ __global__ void faddeeva_kernel(const float* __restrict__ v, const float* __rest
                                 float* __restrict__ H, float* __restrict__ F) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    float wr, wi;
-    faddeeva32(v[i], fad_const(a[i]), wr, wi);
-    H[i] = wr; F[i] = wi;
+    f2 wr, wi;
+    faddeeva_pair(make_float2(v[i], i + 1 < n ? v[i + 1] : v[i]), fad_const(a[i]), wr, wi);   // pair (i, i+1) at a[i]
+    H[i] = wr.x; F[i] = wi.x;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -278,7 +302,7 @@ __global__ void faddeeva_kernel(const float* __restrict__ v, const float* __rest
 static inline unsigned grid_for(int64_t n) { return (unsigned)(n < 0x7fffffffLL ? n : 0x7fffffffLL); }
 
 static inline size_t ga_smem_bytes(int L, int pop) {
-    return (size_t)16 * L + (size_t)2 * pop * ME_NPAR * 4 + (size_t)2 * pop * 4 + 64 * 4;
+    return (size_t)32 * ((L + 1) / 2) + (size_t)2 * pop * ME_NPAR * 4 + (size_t)2 * pop * 4 + 64 * 4;
 }
 
 template <int NL, bool TRIPLET, int THREADS, int MINB>
@@ -296,7 +320,7 @@ template <int NL, bool TRIPLET, int THREADS, int MINB>
 static cudaError_t launch_ga_fitness_t(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs,
                                        const float* mu, int64_t N, float* chi2_out, cudaStream_t st) {
     auto k = ga_fitness_kernel<NL, TRIPLET, THREADS, MINB>;
-    const size_t smem = (size_t)16 * sd.L;
+    const size_t smem = (size_t)32 * ((sd.L + 1) / 2);
     k<<<grid_for(N), THREADS, smem, st>>>(sd, gd, genes, obs, mu, N, chi2_out);
     return cudaGetLastError();
 }
