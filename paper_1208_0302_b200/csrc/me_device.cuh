@@ -191,9 +191,20 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const SynthDesc& d
     if (TRIPLET) {
         const float gvB = d.line[l].g * vB;
         f2 w0r, w0i, w1r, w1i, w2r, w2i;
-        faddeeva_pair(v, fad, w0r, w0i);
-        faddeeva_pair(add2(v, bc(gvB)), fad, w1r, w1i);      // sigma_blue sits at v = -g vB
-        faddeeva_pair(add2(v, bc(-gvB)), fad, w2r, w2i);     // sigma_red  sits at v = +g vB
+        const f2 vb = add2(v, bc(gvB)), vr = add2(v, bc(-gvB));   // sigma_blue sits at v = -g vB, sigma_red at +g vB
+        const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
+        const float rmin = fminf(fminf(fminf(r2p.x, r2p.y), fminf(r2b.x, r2b.y)), fminf(r2r.x, r2r.y));
+        if (rmin >= FAD_CUT2) {
+            // all six arguments in the wing region (the common case): three independent straight-line
+            // evaluations that the scheduler can interleave
+            faddeeva_wing(v, r2p, fad, w0r, w0i);
+            faddeeva_wing(vb, r2b, fad, w1r, w1i);
+            faddeeva_wing(vr, r2r, fad, w2r, w2i);
+        } else {
+            faddeeva_pair(v, fad, w0r, w0i);
+            faddeeva_pair(vb, fad, w1r, w1i);
+            faddeeva_pair(vr, fad, w2r, w2i);
+        }
         pr = fma2(r, w0r, pr); pi = fma2(r, w0i, pi);
         br = fma2(r, w1r, br); bi = fma2(r, w1i, bi);
         rr = fma2(r, w2r, rr); ri = fma2(r, w2i, ri);

@@ -106,35 +106,31 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         __syncthreads();                                   // previous pixel's shared memory is no longer read
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
 
-        // generation 0 (reading G2)
+        // generations 0..G with ONE fitness call site (keeps the loop body inside the instruction cache)
         float g[ME_NPAR];
         float f = INF;
-        int cur = 0;
+        int cur = 1;                                       // generation t reads buffer cur, writes cur ^ 1
         const bool alive = tid < pop;
-        if (alive) {
-            init_genes(g, pixel, (uint32_t)tid, gd);
-#pragma unroll
-            for (int j = 0; j < ME_NPAR; ++j) genes_s[tid * ME_NPAR + j] = g[j];
-        }
-        __syncthreads();
-        if (alive) { f = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s)); chi2_s[tid] = f; }
-        __syncthreads();
-
-        for (int t = 1; t <= gd.generations; ++t) {
-            float fe; int ie;
-            block_argmin(f, tid, scratch, fe, ie);         // elite of generation t-1
+        for (int t = 0; t <= gd.generations; ++t) {
+            float fe = INF; int ie = 0;
+            if (t > 0) block_argmin(f, tid, scratch, fe, ie);   // elite of generation t-1
+            else __syncthreads();                          // obs staged
             const float* gprev = genes_s + cur * pop * ME_NPAR;
             const float* fprev = chi2_s + cur * pop;
             float* gnext = genes_s + (cur ^ 1) * pop * ME_NPAR;
             if (alive) {
-                if (tid == 0) {
+                bool evaluate = true;
+                if (t == 0) {
+                    init_genes(g, pixel, (uint32_t)tid, gd);                       // reading G2
+                } else if (tid == 0) {
 #pragma unroll
                     for (int j = 0; j < ME_NPAR; ++j) g[j] = gprev[ie * ME_NPAR + j];
                     f = fe;                                // carried, not re-evaluated (reading G3)
+                    evaluate = false;
                 } else {
                     make_child(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
-                    f = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
                 }
+                if (evaluate) f = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
 #pragma unroll
                 for (int j = 0; j < ME_NPAR; ++j) gnext[tid * ME_NPAR + j] = g[j];
                 chi2_s[(cur ^ 1) * pop + tid] = f;
