@@ -99,6 +99,8 @@ MEDEV FadConst fad_const(float a) {
     return f;
 }
 
+// FAR = true: |z|^2 >= FAD_FAR2, series truncated after q^3 (next term 3.7/|z|^8 < 1e-8 relative).
+template <bool FAR>
 MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
     const f2 r = rcp2(r2);                                    // 1/|z|^2
     const f2 rr = mul2(r, r);                                 // 1/|z|^4 = |q|^2
@@ -106,12 +108,19 @@ MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
     const f2 qr = mul2(fma2(v, v, -f.a2), rr);                // Re q = (v^2 - a^2)/|z|^4
     const f2 nqi = mul2(mul2(f.two_a, v), rr);                // -Im q = 2 v a/|z|^4
     const f2 t = add2(qr, qr);
-    const f2 b5 = fma2(t, bc(FAD_C6), FAD_C5);
-    const f2 b4 = fma2(t, b5, fma2(m, bc(FAD_C6), FAD_C4));
-    ME_REC(b3, FAD_C3, b4, b5);
-    ME_REC(b2, FAD_C2, b3, b4);
-    ME_REC(b1, FAD_C1, b2, b3);
-    ME_REC(b0, FAD_C0, b1, b2);
+    f2 b0, b1;
+    if (FAR) {
+        const f2 b2 = fma2(t, bc(FAD_C3), FAD_C2);
+        b1 = fma2(t, b2, fma2(m, bc(FAD_C3), FAD_C1));
+        b0 = fma2(t, b1, fma2(m, b2, FAD_C0));
+    } else {
+        const f2 b5 = fma2(t, bc(FAD_C6), FAD_C5);
+        const f2 b4 = fma2(t, b5, fma2(m, bc(FAD_C6), FAD_C4));
+        ME_REC(b3, FAD_C3, b4, b5);
+        ME_REC(b2, FAD_C2, b3, b4);
+        b1 = fma2(t, b2, fma2(m, b3, FAD_C1));
+        b0 = fma2(t, b1, fma2(m, b2, FAD_C0));
+    }
     const f2 Rr = fma2(neg(b1), qr, b0);                      // Re R
     const f2 nRi = mul2(b1, nqi);                             // -Im R
     // w = i s R = r (a + i v)(Rr + i Ri)
@@ -138,7 +147,7 @@ MEDEV void faddeeva_core(f2 v, const FadConst& f, f2& wr, f2& wi) {
 MEDEV void faddeeva_pair(f2 v, const FadConst& f, f2& wr, f2& wi) {
     const f2 r2 = fma2(v, v, f.a2);
     const bool w0 = r2.x >= FAD_CUT2, w1 = r2.y >= FAD_CUT2;
-    if (w0 || w1) faddeeva_wing(v, r2, f, wr, wi);
+    if (w0 || w1) faddeeva_wing<false>(v, r2, f, wr, wi);
     if (!(w0 && w1)) {
         f2 cr, ci;
         faddeeva_core(v, f, cr, ci);
@@ -194,12 +203,17 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const SynthDesc& d
         const f2 vb = add2(v, bc(gvB)), vr = add2(v, bc(-gvB));   // sigma_blue sits at v = -g vB, sigma_red at +g vB
         const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
         const float rmin = fminf(fminf(fminf(r2p.x, r2p.y), fminf(r2b.x, r2b.y)), fminf(r2r.x, r2r.y));
-        if (rmin >= FAD_CUT2) {
-            // all six arguments in the wing region (the common case): three independent straight-line
-            // evaluations that the scheduler can interleave
-            faddeeva_wing(v, r2p, fad, w0r, w0i);
-            faddeeva_wing(vb, r2b, fad, w1r, w1i);
-            faddeeva_wing(vr, r2r, fad, w2r, w2i);
+        if (rmin >= FAD_FAR2) {
+            // all six arguments far from the line: short series
+            faddeeva_wing<true>(v, r2p, fad, w0r, w0i);
+            faddeeva_wing<true>(vb, r2b, fad, w1r, w1i);
+            faddeeva_wing<true>(vr, r2r, fad, w2r, w2i);
+        } else if (rmin >= FAD_CUT2) {
+            // all six arguments in the wing region: three independent straight-line evaluations that the
+            // scheduler can interleave
+            faddeeva_wing<false>(v, r2p, fad, w0r, w0i);
+            faddeeva_wing<false>(vb, r2b, fad, w1r, w1i);
+            faddeeva_wing<false>(vr, r2r, fad, w2r, w2i);
         } else {
             faddeeva_pair(v, fad, w0r, w0i);
             faddeeva_pair(vb, fad, w1r, w1i);
