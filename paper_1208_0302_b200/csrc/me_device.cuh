@@ -351,4 +351,22 @@ __device__ __forceinline__ void make_child(float* child, const float* genes, con
     }
 }
 
+// Block-wide argmin of (value, index) with ties -> lowest index. Values must be >= 0 or +Inf.
+// scratch: 2 * 32 words of shared memory. Every thread returns the same (value, index).
+__device__ __forceinline__ void block_argmin(float v, int idx, uint32_t* scratch, float& vmin, int& imin) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    uint32_t bits = __float_as_uint(v);
+    uint32_t m = __reduce_min_sync(0xffffffffu, bits);
+    uint32_t i = __reduce_min_sync(0xffffffffu, bits == m ? (uint32_t)idx : 0xffffffffu);
+    if (lane == 0) { scratch[warp] = m; scratch[32 + warp] = i; }
+    __syncthreads();
+    const uint32_t mb = lane < nwarps ? scratch[lane] : 0xffffffffu;
+    const uint32_t ib = lane < nwarps ? scratch[32 + lane] : 0xffffffffu;
+    m = __reduce_min_sync(0xffffffffu, mb);
+    i = __reduce_min_sync(0xffffffffu, mb == m ? ib : 0xffffffffu);
+    vmin = __uint_as_float(m);
+    imin = (int)i;
+    __syncthreads();          // scratch may be reused by the next call
+}
+
 }  // namespace me

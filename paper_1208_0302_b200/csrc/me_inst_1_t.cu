@@ -1,0 +1,5 @@
+// Specialisation: 1 line(s), effective triplets.
+#define ME_INST_NL 1
+#define ME_INST_TRIPLET true
+#define ME_INST_TAG t
+#include "me_inst.cuh"

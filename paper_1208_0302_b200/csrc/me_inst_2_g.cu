@@ -1,0 +1,5 @@
+// Specialisation: 2 line(s), general Zeeman component lists.
+#define ME_INST_NL 2
+#define ME_INST_TRIPLET false
+#define ME_INST_TAG g
+#include "me_inst.cuh"

@@ -1,4 +1,5 @@
-// me_kernels.cu — CUDA kernels of libme_b200.so (sm_100a) and their launchers.
+// me_kernels.cu — small kernels (GA hooks, Philox, Faddeeva hook) and the launch dispatch of libme_b200.so (sm_100a).
+// The heavy template kernels are in me_inst.cuh:
 //
 //   ga_invert_kernel   CTA = one pixel, thread = one individual; the whole GA of Alg. 1 runs
 //                      on-chip: observation staged once in shared memory, population double-buffered in shared
@@ -15,222 +16,8 @@
 namespace me {
 
 // ------------------------------------------------------------------------------------------------------------
-// Fitness of one individual held in registers: decode -> per-individual constants -> wavelength loop.
-// obs_s: shared memory, per wavelength pair two float4 = (I0,I1,Q0,Q1), (U0,U1,V0,V1) (broadcast reads, conflict-free).
-// ------------------------------------------------------------------------------------------------------------
-template <int NL, bool TRIPLET>
-__device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
-                                         const float4* obs_s) {
-    float p[ME_NPAR];
-#pragma unroll
-    for (int j = 0; j < ME_NPAR; ++j) p[j] = decode_gene(g[j], gd, j);
-    Individual<NL> ind;
-    setup_individual<NL>(ind, p, mu, sd);
-    f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
-    const int L = sd.L, npair = L >> 1;
-    for (int jp = 0; jp < npair; ++jp) {
-        f2 I, Q, U, V;
-        stokes_pair<NL, TRIPLET>(ind, sd, 2 * jp, false, I, Q, U, V);
-        const float4 o0 = obs_s[2 * jp], o1 = obs_s[2 * jp + 1];           // (I0,I1,Q0,Q1), (U0,U1,V0,V1)
-        const f2 dI = sub2(make_float2(o0.x, o0.y), I), dQ = sub2(make_float2(o0.z, o0.w), Q);
-        const f2 dU = sub2(make_float2(o1.x, o1.y), U), dV = sub2(make_float2(o1.z, o1.w), V);
-        aI = fma2(dI, dI, aI); aQ = fma2(dQ, dQ, aQ); aU = fma2(dU, dU, aU); aV = fma2(dV, dV, aV);
-    }
-    if (L & 1) {                                                            // odd tail: second half is a duplicate, dropped
-        f2 I, Q, U, V;
-        stokes_pair<NL, TRIPLET>(ind, sd, L - 1, true, I, Q, U, V);
-        const float4 o0 = obs_s[2 * npair], o1 = obs_s[2 * npair + 1];
-        const float dI = o0.x - I.x, dQ = o0.z - Q.x, dU = o1.x - U.x, dV = o1.z - V.x;
-        aI.x = fmaf(dI, dI, aI.x); aQ.x = fmaf(dQ, dQ, aQ.x); aU.x = fmaf(dU, dU, aU.x); aV.x = fmaf(dV, dV, aV.x);
-    }
-    const float sI = aI.x + aI.y, sQ = aQ.x + aQ.y, sU = aU.x + aU.y, sV = aV.x + aV.y;
-    float chi2 = gd.inv_nu * fmaf(gd.w2[0], sI, fmaf(gd.w2[1], sQ, fmaf(gd.w2[2], sU, gd.w2[3] * sV)));
-    if (!(chi2 < __int_as_float(0x7f800000))) chi2 = __int_as_float(0x7f800000);   // NaN / Inf -> +Inf (reading G4)
-    return chi2;
-}
-
-// Stage obs[n] ([4][L] in HBM, rows contiguous => coalesced) into shared memory, pair-interleaved:
-// element (s, j) -> word 8 (j/2) + 2 s + (j & 1).  Shared size: 8 * ceil(L/2) floats.
-__device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int L, int tid, int nthreads) {
-    for (int k = tid; k < 4 * L; k += nthreads) {
-        const int s = k / L, j = k - s * L;
-        obs_s[8 * (j >> 1) + 2 * s + (j & 1)] = __ldg(obs_n + k);
-    }
-}
-
-// Block-wide argmin of (value, index) with ties -> lowest index. Values must be >= 0 or +Inf.
-// scratch: 2 * 32 words of shared memory. Every thread returns the same (value, index).
-__device__ __forceinline__ void block_argmin(float v, int idx, uint32_t* scratch, float& vmin, int& imin) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    uint32_t bits = __float_as_uint(v);
-    uint32_t m = __reduce_min_sync(0xffffffffu, bits);
-    uint32_t i = __reduce_min_sync(0xffffffffu, bits == m ? (uint32_t)idx : 0xffffffffu);
-    if (lane == 0) { scratch[warp] = m; scratch[32 + warp] = i; }
-    __syncthreads();
-    const uint32_t mb = lane < nwarps ? scratch[lane] : 0xffffffffu;
-    const uint32_t ib = lane < nwarps ? scratch[32 + lane] : 0xffffffffu;
-    m = __reduce_min_sync(0xffffffffu, mb);
-    i = __reduce_min_sync(0xffffffffu, mb == m ? ib : 0xffffffffu);
-    vmin = __uint_as_float(m);
-    imin = (int)i;
-    __syncthreads();          // scratch may be reused by the next call
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// The fused GA inversion kernel.
-// Dynamic shared memory: obs_s [ceil(L/2)] 2 x float4 | genes [2][pop][9] | chi2 [2][pop] | scratch [64]
-// ------------------------------------------------------------------------------------------------------------
-template <int NL, bool TRIPLET, int THREADS, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB)
-ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
-                 const float* __restrict__ obs, const uint8_t* __restrict__ mask, const float* __restrict__ mu_arr,
-                 int64_t N, float* __restrict__ out_params, float* __restrict__ out_chi2) {
-    extern __shared__ float4 smem4[];
-    const int L = sd.L, pop = gd.pop;
-    float* obs_s = reinterpret_cast<float*>(smem4);
-    float* genes_s = obs_s + 8 * ((L + 1) >> 1);
-    float* chi2_s = genes_s + 2 * pop * ME_NPAR;
-    uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + 2 * pop);
-    const int tid = threadIdx.x;
-    const float INF = __int_as_float(0x7f800000);
-
-    for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
-        if (mask != nullptr && mask[n] == 0) {
-            const float qnan = __int_as_float(0x7fc00000);
-            if (tid < ME_NPAR) out_params[n * ME_NPAR + tid] = qnan;
-            if (tid == 0) out_chi2[n] = qnan;
-            continue;
-        }
-        const uint32_t pixel = gd.pixel_base + (uint32_t)n;
-        const float mu = mu_arr != nullptr ? __ldg(mu_arr + n) : 1.0f;
-        __syncthreads();                                   // previous pixel's shared memory is no longer read
-        stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
-
-        // generations 0..G with ONE fitness call site (keeps the loop body inside the instruction cache)
-        float g[ME_NPAR];
-        float f = INF;
-        int cur = 1;                                       // generation t reads buffer cur, writes cur ^ 1
-        const bool alive = tid < pop;
-        for (int t = 0; t <= gd.generations; ++t) {
-            float fe = INF; int ie = 0;
-            if (t > 0) block_argmin(f, tid, scratch, fe, ie);   // elite of generation t-1
-            else __syncthreads();                          // obs staged
-            const float* gprev = genes_s + cur * pop * ME_NPAR;
-            const float* fprev = chi2_s + cur * pop;
-            float* gnext = genes_s + (cur ^ 1) * pop * ME_NPAR;
-            if (alive) {
-                bool evaluate = true;
-                if (t == 0) {
-                    init_genes(g, pixel, (uint32_t)tid, gd);                       // reading G2
-                } else if (tid == 0) {
-#pragma unroll
-                    for (int j = 0; j < ME_NPAR; ++j) g[j] = gprev[ie * ME_NPAR + j];
-                    f = fe;                                // carried, not re-evaluated (reading G3)
-                    evaluate = false;
-                } else {
-                    make_child(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
-                }
-                if (evaluate) f = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
-#pragma unroll
-                for (int j = 0; j < ME_NPAR; ++j) gnext[tid * ME_NPAR + j] = g[j];
-                chi2_s[(cur ^ 1) * pop + tid] = f;
-            }
-            cur ^= 1;
-            __syncthreads();
-        }
-
-        float fe; int ie;
-        block_argmin(f, tid, scratch, fe, ie);             // reading G5
-        if (tid == ie) {
-#pragma unroll
-            for (int j = 0; j < ME_NPAR; ++j) out_params[n * ME_NPAR + j] = decode_gene(g[j], gd, j);
-            out_chi2[n] = f;
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// me_synth: warp = parameter vector, lane = wavelength pair.  out_stokes[P,4,L]: each (vector, Stokes) row is
-// written as consecutive 128-byte warp stores.  chi2 (optional) is reduced with warp shuffles.
-// ------------------------------------------------------------------------------------------------------------
-template <int NL, bool TRIPLET>
-__global__ void __launch_bounds__(256)
-me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
-                int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
-                float w2I, float w2Q, float w2U, float w2V, float inv_nu, float* __restrict__ out_chi2) {
-    const int lane = threadIdx.x & 31;
-    const int64_t warp0 = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    const int64_t nwarps = (int64_t)gridDim.x * (blockDim.x >> 5);
-    const int L = sd.L;
-    for (int64_t v = warp0; v < P; v += nwarps) {
-        float p[ME_NPAR];
-#pragma unroll
-        for (int j = 0; j < ME_NPAR; ++j) p[j] = __ldg(params + v * ME_NPAR + j);
-        const float mu = mu_arr != nullptr ? __ldg(mu_arr + v) : 1.0f;
-        Individual<NL> ind;
-        setup_individual<NL>(ind, p, mu, sd);
-        float acc = 0.f;
-        float* o = out_stokes != nullptr ? out_stokes + v * 4 * (int64_t)L : nullptr;
-        const bool even = (L & 1) == 0;                      // float2 rows are 8-byte aligned only for even L
-        for (int j = 2 * lane; j < L; j += 64) {
-            const bool tail = j + 1 >= L;
-            f2 I, Q, U, V;
-            stokes_pair<NL, TRIPLET>(ind, sd, j, tail, I, Q, U, V);
-            if (o != nullptr) {
-                if (even) {
-                    __stcs(reinterpret_cast<float2*>(o + j), I); __stcs(reinterpret_cast<float2*>(o + L + j), Q);
-                    __stcs(reinterpret_cast<float2*>(o + 2 * L + j), U); __stcs(reinterpret_cast<float2*>(o + 3 * L + j), V);
-                } else {
-                    __stcs(o + j, I.x); __stcs(o + L + j, Q.x); __stcs(o + 2 * L + j, U.x); __stcs(o + 3 * L + j, V.x);
-                    if (!tail) { __stcs(o + j + 1, I.y); __stcs(o + L + j + 1, Q.y); __stcs(o + 2 * L + j + 1, U.y); __stcs(o + 3 * L + j + 1, V.y); }
-                }
-            }
-            if (out_chi2 != nullptr) {
-                const float dI = __ldg(obs_ref + j) - I.x, dQ = __ldg(obs_ref + L + j) - Q.x;
-                const float dU = __ldg(obs_ref + 2 * L + j) - U.x, dV = __ldg(obs_ref + 3 * L + j) - V.x;
-                acc = fmaf(w2I * dI, dI, acc); acc = fmaf(w2Q * dQ, dQ, acc);
-                acc = fmaf(w2U * dU, dU, acc); acc = fmaf(w2V * dV, dV, acc);
-                if (!tail) {
-                    const float eI = __ldg(obs_ref + j + 1) - I.y, eQ = __ldg(obs_ref + L + j + 1) - Q.y;
-                    const float eU = __ldg(obs_ref + 2 * L + j + 1) - U.y, eV = __ldg(obs_ref + 3 * L + j + 1) - V.y;
-                    acc = fmaf(w2I * eI, eI, acc); acc = fmaf(w2Q * eQ, eQ, acc);
-                    acc = fmaf(w2U * eU, eU, acc); acc = fmaf(w2V * eV, eV, acc);
-                }
-            }
-        }
-        if (out_chi2 != nullptr) {
-#pragma unroll
-            for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
-            if (lane == 0) out_chi2[v] = acc * inv_nu;
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------------
 // Test hooks
 // ------------------------------------------------------------------------------------------------------------
-template <int NL, bool TRIPLET, int THREADS, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB)
-ga_fitness_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
-                  const float* __restrict__ genes, const float* __restrict__ obs, const float* __restrict__ mu_arr,
-                  int64_t N, float* __restrict__ chi2_out) {
-    extern __shared__ float4 smem4[];
-    float* obs_s = reinterpret_cast<float*>(smem4);
-    const int L = sd.L, pop = gd.pop, tid = threadIdx.x;
-    for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
-        __syncthreads();
-        stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
-        __syncthreads();
-        if (tid < pop) {
-            float g[ME_NPAR];
-#pragma unroll
-            for (int j = 0; j < ME_NPAR; ++j) g[j] = genes[(n * pop + tid) * ME_NPAR + j];
-            const float mu = mu_arr != nullptr ? __ldg(mu_arr + n) : 1.0f;
-            chi2_out[n * pop + tid] = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
-        }
-    }
-}
-
 // One generation from given genes and given fitness (shared: genes [pop][9] | chi2 [pop] | scratch [64]).
 __global__ void ga_step_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ genes_in,
                                const float* __restrict__ chi2_in, int64_t N, int t, float* __restrict__ genes_out) {
@@ -297,62 +84,41 @@ __global__ void faddeeva_kernel(const float* __restrict__ v, const float* __rest
 // ------------------------------------------------------------------------------------------------------------
 static inline unsigned grid_for(int64_t n) { return (unsigned)(n < 0x7fffffffLL ? n : 0x7fffffffLL); }
 
-static inline size_t ga_smem_bytes(int L, int pop) {
-    return (size_t)32 * ((L + 1) / 2) + (size_t)2 * pop * ME_NPAR * 4 + (size_t)2 * pop * 4 + 64 * 4;
-}
+// The heavy kernels live in me_inst_<nl>_<t|g>.cu (one translation unit per specialisation).
+#define ME_DECL_INST(NL, TAG)                                                                                            \
+    cudaError_t launch_ga_invert_##NL##_##TAG(const SynthDesc&, const GaDesc&, const float*, const uint8_t*, const float*, \
+                                              int64_t, float*, float*, cudaStream_t);                                     \
+    cudaError_t launch_ga_fitness_##NL##_##TAG(const SynthDesc&, const GaDesc&, const float*, const float*, const float*,  \
+                                               int64_t, float*, cudaStream_t);                                            \
+    cudaError_t launch_synth_##NL##_##TAG(const SynthDesc&, const float*, const float*, int64_t, float*, const float*,    \
+                                          const float*, float, float*, cudaStream_t);
+ME_DECL_INST(1, t) ME_DECL_INST(2, t) ME_DECL_INST(4, t) ME_DECL_INST(1, g) ME_DECL_INST(2, g) ME_DECL_INST(4, g)
 
-template <int NL, bool TRIPLET, int THREADS, int MINB>
-static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask,
-                                      const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
-    auto k = ga_invert_kernel<NL, TRIPLET, THREADS, MINB>;
-    const size_t smem = ga_smem_bytes(sd.L, gd.pop);
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    k<<<grid_for(N), THREADS, smem, st>>>(sd, gd, obs, mask, mu, N, out_params, out_chi2);
-    return cudaGetLastError();
-}
-
-template <int NL, bool TRIPLET, int THREADS, int MINB>
-static cudaError_t launch_ga_fitness_t(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs,
-                                       const float* mu, int64_t N, float* chi2_out, cudaStream_t st) {
-    auto k = ga_fitness_kernel<NL, TRIPLET, THREADS, MINB>;
-    const size_t smem = (size_t)32 * ((sd.L + 1) / 2);
-    k<<<grid_for(N), THREADS, smem, st>>>(sd, gd, genes, obs, mu, N, chi2_out);
-    return cudaGetLastError();
-}
-
-// (pop -> block size, min blocks/SM) keeps the fitness loop at <= 128 registers/thread where the block allows it.
-#define ME_DISPATCH_THREADS(FN, NL, TR, ...)                                                       \
-    do {                                                                                            \
-        const int pop_ = gd.pop;                                                                    \
-        if (pop_ <= 64) return FN<NL, TR, 64, 8>(__VA_ARGS__);                                      \
-        if (pop_ <= 128) return FN<NL, TR, 128, 4>(__VA_ARGS__);                                    \
-        if (pop_ <= 256) return FN<NL, TR, 256, 2>(__VA_ARGS__);                                    \
-        if (pop_ <= 512) return FN<NL, TR, 512, 1>(__VA_ARGS__);                                    \
-        return FN<NL, TR, 1024, 1>(__VA_ARGS__);                                                    \
-    } while (0)
-
-#define ME_DISPATCH(FN, ...)                                                                        \
-    do {                                                                                            \
-        if (sd.all_triplets) {                                                                      \
-            if (sd.n_lines == 1) ME_DISPATCH_THREADS(FN, 1, true, __VA_ARGS__);                     \
-            if (sd.n_lines == 2) ME_DISPATCH_THREADS(FN, 2, true, __VA_ARGS__);                     \
-            ME_DISPATCH_THREADS(FN, ME_MAX_LINES, true, __VA_ARGS__);                               \
-        } else {                                                                                    \
-            if (sd.n_lines == 1) ME_DISPATCH_THREADS(FN, 1, false, __VA_ARGS__);                    \
-            if (sd.n_lines == 2) ME_DISPATCH_THREADS(FN, 2, false, __VA_ARGS__);                    \
-            ME_DISPATCH_THREADS(FN, ME_MAX_LINES, false, __VA_ARGS__);                              \
-        }                                                                                           \
+#define ME_DISPATCH(BASE, ...)                                                       \
+    do {                                                                             \
+        if (sd.all_triplets) {                                                       \
+            if (sd.n_lines == 1) return BASE##_1_t(__VA_ARGS__);                     \
+            if (sd.n_lines == 2) return BASE##_2_t(__VA_ARGS__);                     \
+            return BASE##_4_t(__VA_ARGS__);                                          \
+        }                                                                            \
+        if (sd.n_lines == 1) return BASE##_1_g(__VA_ARGS__);                         \
+        if (sd.n_lines == 2) return BASE##_2_g(__VA_ARGS__);                         \
+        return BASE##_4_g(__VA_ARGS__);                                              \
     } while (0)
 
 cudaError_t launch_ga_invert(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask, const float* mu,
                              int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
-    ME_DISPATCH(launch_ga_invert_t, sd, gd, obs, mask, mu, N, out_params, out_chi2, st);
+    ME_DISPATCH(launch_ga_invert, sd, gd, obs, mask, mu, N, out_params, out_chi2, st);
 }
 
 cudaError_t launch_ga_fitness(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs, const float* mu,
                               int64_t N, float* chi2_out, cudaStream_t st) {
-    ME_DISPATCH(launch_ga_fitness_t, sd, gd, genes, obs, mu, N, chi2_out, st);
+    ME_DISPATCH(launch_ga_fitness, sd, gd, genes, obs, mu, N, chi2_out, st);
+}
+
+cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* mu, int64_t P, float* out_stokes,
+                         const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, cudaStream_t st) {
+    ME_DISPATCH(launch_synth, sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
 }
 
 cudaError_t launch_ga_step(const GaDesc& gd, const float* genes_in, const float* chi2_in, int64_t N, int t,
@@ -367,32 +133,6 @@ cudaError_t launch_ga_init(const GaDesc& gd, int64_t N, float* genes_out, cudaSt
     const int64_t total = N * gd.pop;
     ga_init_kernel<<<grid_for((total + 255) / 256), 256, 0, st>>>(gd, N, genes_out);
     return cudaGetLastError();
-}
-
-template <int NL, bool TRIPLET>
-static cudaError_t launch_synth_t(const SynthDesc& sd, const float* params, const float* mu, int64_t P, float* out_stokes,
-                                  const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, cudaStream_t st) {
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int64_t blocks_needed = (P + 7) / 8;                       // 8 warps per block
-    const int64_t cap = (int64_t)sms * 8;                            // persistent grid: 8 resident blocks per SM
-    const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
-    me_synth_kernel<NL, TRIPLET><<<grid, 256, 0, st>>>(sd, params, mu, P, out_stokes, obs_ref, w2[0], w2[1], w2[2], w2[3],
-                                                       inv_nu, out_chi2);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* mu, int64_t P, float* out_stokes,
-                         const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, cudaStream_t st) {
-    if (sd.all_triplets) {
-        if (sd.n_lines == 1) return launch_synth_t<1, true>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
-        if (sd.n_lines == 2) return launch_synth_t<2, true>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
-        return launch_synth_t<ME_MAX_LINES, true>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
-    }
-    if (sd.n_lines == 1) return launch_synth_t<1, false>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
-    if (sd.n_lines == 2) return launch_synth_t<2, false>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
-    return launch_synth_t<ME_MAX_LINES, false>(sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
 }
 
 cudaError_t launch_philox(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3, int64_t n,
