@@ -85,69 +85,66 @@ MEDEV f2 rcp2(f2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
 
 // ------------------------------------------------------------------------------------------------------------
 // Faddeeva function w(v + i a) = H + iF on a pair of v, FP32, two regions.
-//   wing |z|^2 >= CUT2: w = (i/sqrt(pi)) s R(q), s = 1/z, q = s^2, R = asymptotic series to q^6.  H comes out as
+//   wing |z|^2 >= CUT2: w = (i/sqrt(pi)) s R(q), s = 1/z, q = s^2, R = asymptotic series to q^5 (q^3, q^2 farther out).  H comes out as
 //                       a/(sqrt(pi)|z|^2) x (1 + ...): no cancellation, full relative accuracy.
 //   core |z|^2 <  CUT2: Weideman (1994), N = FAD_N terms in Z = (L + iz)/(L - iz).
 // ------------------------------------------------------------------------------------------------------------
-struct FadConst { float a, a2, two_a, La, La2, Lma2; };
+struct FadConst { float a, a2, m4a2, La, Lma, La2, Lma2, t4LLa; };
 
 MEDEV FadConst fad_const(float a) {
     FadConst f;
-    f.a = a; f.a2 = a * a; f.two_a = 2.0f * a;
-    f.La = FAD_L + a; f.La2 = f.La * f.La;
-    f.Lma2 = (FAD_L - a) * (FAD_L - a);
+    f.a = a; f.a2 = a * a; f.m4a2 = -4.0f * f.a2;
+    f.La = FAD_L + a; f.Lma = FAD_L - a; f.La2 = f.La * f.La; f.Lma2 = f.Lma * f.Lma;
+    f.t4LLa = 2.0f * FAD_2L * f.La;
     return f;
 }
 
-// FAR = true: |z|^2 >= FAD_FAR2, series truncated after q^3 (next term 3.7/|z|^8 < 1e-8 relative).
-template <bool FAR>
+// Wing region.  With t = 2 Re q, m = -|q|^2 the recurrence gives R(q) = b0 - b1 conj(q); since s conj(q) = |s|^2 conj(s)
+// and |s|^2 = r = 1/|z|^2:   w = i s R = r [ a (b0 + r b1) + i v (b0 - r b1) ]   (no cancellation in H).
+// K = number of series terms beyond the leading one: 5 for |z| >= FAD_CUT, 3 for >= FAD_MID, 2 for >= FAD_FAR.
+template <int K>
 MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
     const f2 r = rcp2(r2);                                    // 1/|z|^2
-    const f2 rr = mul2(r, r);                                 // 1/|z|^4 = |q|^2
-    const f2 m = neg(rr);                                     // -|q|^2
-    const f2 qr = mul2(fma2(v, v, -f.a2), rr);                // Re q = (v^2 - a^2)/|z|^4
-    const f2 nqi = mul2(mul2(f.two_a, v), rr);                // -Im q = 2 v a/|z|^4
-    const f2 t = add2(qr, qr);
+    const f2 t = mul2(fma2(f.m4a2, r, 2.0f), r);              // 2 Re q = 2 (v^2 - a^2)/|z|^4 = (2 - 4 a^2 r) r
+    const f2 m = mul2(neg(r), r);                             // -|q|^2 = -1/|z|^4
     f2 b0, b1;
-    if (FAR) {
+    if (K == 2) {
+        b1 = fma2(t, bc(FAD_C2), FAD_C1);
+        b0 = fma2(t, b1, fma2(m, bc(FAD_C2), FAD_C0));
+    } else if (K == 3) {
         const f2 b2 = fma2(t, bc(FAD_C3), FAD_C2);
         b1 = fma2(t, b2, fma2(m, bc(FAD_C3), FAD_C1));
         b0 = fma2(t, b1, fma2(m, b2, FAD_C0));
     } else {
-        const f2 b5 = fma2(t, bc(FAD_C6), FAD_C5);
-        const f2 b4 = fma2(t, b5, fma2(m, bc(FAD_C6), FAD_C4));
-        ME_REC(b3, FAD_C3, b4, b5);
+        const f2 b4 = fma2(t, bc(FAD_C5), FAD_C4);
+        const f2 b3 = fma2(t, b4, fma2(m, bc(FAD_C5), FAD_C3));
         ME_REC(b2, FAD_C2, b3, b4);
         b1 = fma2(t, b2, fma2(m, b3, FAD_C1));
         b0 = fma2(t, b1, fma2(m, b2, FAD_C0));
     }
-    const f2 Rr = fma2(neg(b1), qr, b0);                      // Re R
-    const f2 nRi = mul2(b1, nqi);                             // -Im R
-    // w = i s R = r (a + i v)(Rr + i Ri)
-    wr = mul2(r, fma2(f.a, Rr, mul2(v, nRi)));
-    wi = mul2(r, fma2(v, Rr, mul2(-f.a, nRi)));
+    wr = mul2(mul2(f.a, r), fma2(r, b1, b0));
+    wi = mul2(mul2(v, r), fma2(neg(r), b1, b0));
 }
 
+// Core region (Weideman).  D = 1/(L - iz) = r ((L+a) + i v), r = 1/|L - iz|^2, Z = (L + iz) D.  With t = 2 Re Z,
+// m = -|Z|^2 the recurrence gives p(Z) = b0 - b1 conj(Z), and conj(Z) D = r conj(L + iz), so
+//   p D = r [ (b0 (L+a) - b1 (L-a)) + i v (b0 + b1) ],     w = D (p D + 1/sqrt(pi)).
 MEDEV void faddeeva_core(f2 v, const FadConst& f, f2& wr, f2& wi) {
     const f2 v2 = mul2(v, v);
     const f2 r = rcp2(add2(v2, bc(f.La2)));                   // 1/|L - iz|^2
-    const f2 dr = mul2(f.La, r), di = mul2(v, r);             // D = 1/(L - iz)
-    const f2 zr = fma2(FAD_2L, dr, -1.0f), zi = mul2(FAD_2L, di);   // Z = (L + iz) D = 2 L D - 1
-    const f2 t = add2(zr, zr);
-    const f2 m = neg(mul2(add2(v2, bc(f.Lma2)), r));          // -|Z|^2 = -|L + iz|^2 / |L - iz|^2
+    const f2 t = fma2(f.t4LLa, r, -2.0f);                     // 2 Re Z = 2 (2 L (L+a) r - 1)
+    const f2 m = mul2(neg(add2(v2, bc(f.Lma2))), r);          // -|Z|^2 = -|L + iz|^2 / |L - iz|^2
     FAD_CORE_RECURRENCE(t, m)
-    const f2 Pr = fma2(neg(cb1), zr, cb0), Pi = mul2(cb1, zi);   // p(Z), the factor 2 folded into the table
-    // w = D (p D + 1/sqrt(pi))
-    const f2 tr = fma2(neg(Pi), di, fma2(Pr, dr, FAD_INV_SQRTPI));
-    const f2 ti = fma2(Pi, dr, mul2(Pr, di));
-    wr = fma2(dr, tr, neg(mul2(di, ti)));
-    wi = fma2(dr, ti, mul2(di, tr));
+    const f2 X = fma2(r, fma2(f.La, cb0, mul2(-f.Lma, cb1)), FAD_INV_SQRTPI);   // Re(p D) + 1/sqrt(pi)
+    const f2 Y = mul2(mul2(r, v), add2(cb0, cb1));                                // Im(p D)
+    wr = mul2(r, fma2(f.La, X, neg(mul2(v, Y))));
+    wi = mul2(r, fma2(f.La, Y, mul2(v, X)));
 }
 
 MEDEV void faddeeva_pair(f2 v, const FadConst& f, f2& wr, f2& wi) {
     const f2 r2 = fma2(v, v, f.a2);
     const bool w0 = r2.x >= FAD_CUT2, w1 = r2.y >= FAD_CUT2;
-    if (w0 || w1) faddeeva_wing<false>(v, r2, f, wr, wi);
+    if (w0 || w1) faddeeva_wing<5>(v, r2, f, wr, wi);
     if (!(w0 && w1)) {
         f2 cr, ci;
         faddeeva_core(v, f, cr, ci);
@@ -203,17 +200,20 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const SynthDesc& d
         const f2 vb = add2(v, bc(gvB)), vr = add2(v, bc(-gvB));   // sigma_blue sits at v = -g vB, sigma_red at +g vB
         const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
         const float rmin = fminf(fminf(fminf(r2p.x, r2p.y), fminf(r2b.x, r2b.y)), fminf(r2r.x, r2r.y));
+        // When all six arguments lie in one wing tier (the common case) the three evaluations are independent
+        // straight-line code that the scheduler interleaves; the series shortens with distance from the line.
         if (rmin >= FAD_FAR2) {
-            // all six arguments far from the line: short series
-            faddeeva_wing<true>(v, r2p, fad, w0r, w0i);
-            faddeeva_wing<true>(vb, r2b, fad, w1r, w1i);
-            faddeeva_wing<true>(vr, r2r, fad, w2r, w2i);
+            faddeeva_wing<2>(v, r2p, fad, w0r, w0i);
+            faddeeva_wing<2>(vb, r2b, fad, w1r, w1i);
+            faddeeva_wing<2>(vr, r2r, fad, w2r, w2i);
+        } else if (rmin >= FAD_MID2) {
+            faddeeva_wing<3>(v, r2p, fad, w0r, w0i);
+            faddeeva_wing<3>(vb, r2b, fad, w1r, w1i);
+            faddeeva_wing<3>(vr, r2r, fad, w2r, w2i);
         } else if (rmin >= FAD_CUT2) {
-            // all six arguments in the wing region: three independent straight-line evaluations that the
-            // scheduler can interleave
-            faddeeva_wing<false>(v, r2p, fad, w0r, w0i);
-            faddeeva_wing<false>(vb, r2b, fad, w1r, w1i);
-            faddeeva_wing<false>(vr, r2r, fad, w2r, w2i);
+            faddeeva_wing<5>(v, r2p, fad, w0r, w0i);
+            faddeeva_wing<5>(vb, r2b, fad, w1r, w1i);
+            faddeeva_wing<5>(vr, r2r, fad, w2r, w2i);
         } else {
             faddeeva_pair(v, fad, w0r, w0i);
             faddeeva_pair(vb, fad, w1r, w1i);
