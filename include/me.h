@@ -125,6 +125,13 @@ int me_philox_many(uint64_t seed, uint32_t c0_base, uint32_t c1, uint32_t c2, ui
 /* Device Faddeeva evaluator alone: w(v + i a) -> (H, F), all device [n] f32. */
 int me_faddeeva(const float* v, const float* a, int64_t n, float* H, float* F, void* stream);
 
+/* Instruction-throughput probe for the roofline denominators (SURVEY.md par. 8(d)): launches `blocks` CTAs of 256
+ * threads, each thread running `iters` x 32 slots of one instruction class in 8 independent register chains.
+ * kind: 0 FFMA, 1 FFMA2 (packed fp32x2), 2 FFMA2+FFMA 1:1, 3 MUFU.RCP, 4 FMUL2, 5 FFMA2+FFMA 2:1, 6 FFMA2+MUFU 8:1,
+ *       7-9 FFMA2 operand forms (pair*scalar+scalar, pair*pair+imm, pair*scalar+pair), 10 FADD2.
+ * out: device [blocks*256] f32 scratch (never written in practice). The caller times the call with CUDA events. */
+int me_peak_probe(int kind, int iters, int blocks, float* out, void* stream);
+
 /* Host-only: Zeeman pattern of an LS-coupling transition, lower/upper = (S, L, J).
  * Fills up to cap entries and returns the number of components (> cap means truncated), or a negative me_status. */
 int me_zeeman_pattern(double S_lo, double L_lo, double J_lo, double S_up, double L_up, double J_up,

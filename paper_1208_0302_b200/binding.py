@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libme_b200.so")
 _lib = None
 
 EXPORTS = ["me_synth", "ga_invert", "ga_step", "ga_fitness", "ga_init", "me_philox", "me_philox_many", "me_faddeeva",
-           "me_zeeman_pattern", "me_strerror", "me_last_cuda_error", "me_version"]
+           "me_zeeman_pattern", "me_peak_probe", "me_strerror", "me_last_cuda_error", "me_version"]
 
 
 class MeError(RuntimeError):
@@ -243,3 +243,12 @@ def me_faddeeva(v, a):
     _check(lib().me_faddeeva(_dev(v, torch.float32, "v"), _dev(a, torch.float32, "a"), C.c_int64(v.numel()),
                              _dev(H, torch.float32, "H"), _dev(F, torch.float32, "F"), _stream()), "me_faddeeva")
     return H, F
+
+
+def me_peak_probe(kind, iters, blocks, scratch):
+    """Launches one instruction-throughput probe (see include/me.h); returns the lane-slot count it executes."""
+    import torch
+    assert scratch.numel() >= blocks * 256
+    _check(lib().me_peak_probe(C.c_int(kind), C.c_int(iters), C.c_int(blocks), _dev(scratch, torch.float32, "out"), _stream()),
+           "me_peak_probe")
+    return blocks * 256 * iters * 32

@@ -227,6 +227,14 @@ int me_faddeeva(const float* v, const float* a, int64_t n, float* H, float* F, v
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 
+int me_peak_probe(int kind, int iters, int blocks, float* out, void* stream) {
+    if (kind < 0 || kind > 10) return ME_ERR_RANGE;
+    if (iters < 1 || blocks < 1) return ME_ERR_SHAPE;
+    if (out == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_probe(kind, iters, blocks, out, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
 // Zeeman pattern in LS coupling: Lande factors, shifts g_l M_l - g_u M_u, dipole strengths per Delta M.
 int me_zeeman_pattern(double S_lo, double L_lo, double J_lo, double S_up, double L_up, double J_up,
                       int cap, float* shift, float* weight, int8_t* kind) {

@@ -126,6 +126,35 @@ MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
     wi = mul2(mul2(v, r), fma2(neg(r), b1, b0));
 }
 
+// Far tier (|z|^2 >= FAD_FAR2, a <= FAD_FAR_AMAX): the K = 2 series rewritten as polynomials in r = 1/|z|^2 alone.
+// With v^2 = 1/r - a^2,  Re/Im of i s (C0 + C1 q + C2 q^2) become
+//   H = a r X(r),  X = C0 + 3 C1 r + (5 C2 - 4 a^2 C1) r^2 - 20 a^2 C2 r^3 + 16 a^4 C2 r^4
+//   F = v r Y(r),  Y = C0 +   C1 r + (  C2 - 4 a^2 C1) r^2 - 12 a^2 C2 r^3 + 16 a^4 C2 r^4
+// (the r^4 terms are < 1e-8 relative for a <= FAD_FAR_AMAX and are dropped).  The coefficients depend on the individual
+// only, so each Horner step is FFMA2 (pair x pair + scalar) -- the full-rate operand form (profiles/r1c peaks: an
+// FFMA2 whose ADDEND is a register pair runs at 0.77 of that rate) -- and the line strength r_l and the factor a are
+// folded into them:  fx = a r_l (x3, x2, x1, C0),  fy = r_l (y3, y2, y1, C0).
+struct FarCoef { float x3, x2, x1, x0, y3, y2, y1, y0; };
+
+MEDEV FarCoef far_coef(float a, float strength) {
+    FarCoef c;
+    const float a2 = a * a, sa = strength * a;
+    c.x0 = sa * FAD_C0; c.x1 = sa * (3.0f * FAD_C1); c.x2 = sa * fmaf(-4.0f * FAD_C1, a2, 5.0f * FAD_C2);
+    c.x3 = sa * (-20.0f * FAD_C2) * a2;
+    c.y0 = strength * FAD_C0; c.y1 = strength * FAD_C1; c.y2 = strength * fmaf(-4.0f * FAD_C1, a2, FAD_C2);
+    c.y3 = strength * (-12.0f * FAD_C2) * a2;
+    return c;
+}
+
+// accumulates r_l w(v + i a) into (sr, si)
+MEDEV void faddeeva_far_acc(f2 v, f2 r2, const FarCoef& c, f2& sr, f2& si) {
+    const f2 r = rcp2(r2);
+    const f2 X = fma2(fma2(fma2(bc(c.x3), r, c.x2), r, c.x1), r, c.x0);
+    const f2 Y = fma2(fma2(fma2(bc(c.y3), r, c.y2), r, c.y1), r, c.y0);
+    sr = fma2(r, X, sr);
+    si = fma2(mul2(v, r), Y, si);
+}
+
 // Core region (Weideman).  D = 1/(L - iz) = r ((L+a) + i v), r = 1/|L - iz|^2, Z = (L + iz) D.  With t = 2 Re Z,
 // m = -|Z|^2 the recurrence gives p(Z) = b0 - b1 conj(Z), and conj(Z) D = r conj(L + iz), so
 //   p D = r [ (b0 (L+a) - b1 (L-a)) + i v (b0 + b1) ],     w = D (p D + 1/sqrt(pi)).
@@ -159,6 +188,8 @@ MEDEV void faddeeva_pair(f2 v, const FadConst& f, f2& wr, f2& wi) {
 template <int NL>
 struct Individual {
     FadConst fad;
+    FarCoef far[NL];                  // far-tier polynomial coefficients per line (strength and a folded in)
+    float far2;                       // |z|^2 threshold of the far tier (+Inf when a > FAD_FAR_AMAX)
     float invD[NL], v0[NL], vB[NL];   // 1/dlambdaD_l, -doppler_l/dlambdaD_l, Zeeman splitting in Doppler units
     float kA, kB, kC;                 // h sin^2(gamma), h (1 + cos^2 gamma)/2, h cos(gamma);  h = eta0 / (2 sqrt(pi))
     float c2x, s2x;                   // cos 2chi, sin 2chi
@@ -176,11 +207,13 @@ MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const
     ind.kB = h * 0.5f * fmaf(cg, cg, 1.0f);
     ind.kC = h * cg;
     ind.fad = fad_const(a);
+    ind.far2 = a <= FAD_FAR_AMAX ? FAD_FAR2 : __int_as_float(0x7f800000);
     ind.S0 = p[7];
     ind.muS1 = mu * p[8];
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
-        if (NL == ME_MAX_LINES && l >= d.n_lines) { ind.invD[l] = ind.v0[l] = ind.vB[l] = 0.f; continue; }
+        if (NL == ME_MAX_LINES && l >= d.n_lines) { ind.invD[l] = ind.v0[l] = ind.vB[l] = 0.f; ind.far[l] = far_coef(a, 0.f); continue; }
+        ind.far[l] = far_coef(a, d.line[l].strength);
         const float inv = 1.0f / (dld * d.line[l].dld_scale);
         ind.invD[l] = inv;
         ind.v0[l] = -(d.line[l].lam0_over_c * vlos) * inv;
@@ -191,7 +224,7 @@ MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const
 // Profile sums of one line at a pair of reduced wavelengths v:
 //   S_kind += r_l * sum_c weight_c * w(v - shift_c vB + i a)
 template <bool TRIPLET>
-MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const SynthDesc& d, int l,
+MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far, float far2, const SynthDesc& d, int l,
                          f2& br, f2& bi, f2& pr, f2& pi, f2& rr, f2& ri) {
     const float r = d.line[l].strength;
     if (TRIPLET) {
@@ -202,7 +235,13 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const SynthDesc& d
         const float rmin = fminf(fminf(fminf(r2p.x, r2p.y), fminf(r2b.x, r2b.y)), fminf(r2r.x, r2r.y));
         // When all six arguments lie in one wing tier (the common case) the three evaluations are independent
         // straight-line code that the scheduler interleaves; the series shortens with distance from the line.
-        if (rmin >= FAD_FAR2) {
+        if (rmin >= far2) {
+            faddeeva_far_acc(v, r2p, far, pr, pi);
+            faddeeva_far_acc(vb, r2b, far, br, bi);
+            faddeeva_far_acc(vr, r2r, far, rr, ri);
+            return;
+        }
+        if (rmin >= FAD_FAR2) {                                   // a > FAD_FAR_AMAX: the series itself
             faddeeva_wing<2>(v, r2p, fad, w0r, w0i);
             faddeeva_wing<2>(vb, r2b, fad, w1r, w1i);
             faddeeva_wing<2>(vr, r2r, fad, w2r, w2i);
@@ -250,7 +289,7 @@ MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bo
         if (NL == ME_MAX_LINES && l >= d.n_lines) break;      // NL == ME_MAX_LINES is the run-time-sized fallback
         const f2 off = tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]);
         const f2 v = fma2(ind.invD[l], off, ind.v0[l]);
-        line_profiles<TRIPLET>(v, ind.vB[l], ind.fad, d, l, br, bi, pr, pi, rr, ri);
+        line_profiles<TRIPLET>(v, ind.vB[l], ind.fad, ind.far[l], ind.far2, d, l, br, bi, pr, pi, rr, ri);
     }
     const f2 sr = add2(br, rr), si = add2(bi, ri);                // sigma sums
     const f2 eI = fma2(ind.kA, pr, fma2(ind.kB, sr, 1.0f));
