@@ -22,10 +22,14 @@ if ROOT not in sys.path:
 
 from paper_1208_0302_b200 import workloads as W  # noqa: E402
 
-# FP32 work per wavelength point of the fused fitness loop, counted from an ncu capture of this workload
-# (profiles/: smsp__sass_thread_inst_executed_op_{ffma,fmul,fadd}_pred_on / lambda-points; FFMA = 2 flop).
-# See DESIGN.md "Roofline".  Keyed by workload name.
-FLOP_PER_POINT = {"config0_tiny": 260.0, "config1_map256": 477.0, "config3_fulldisc": 477.0}
+# FP32 work per wavelength point of the fused fitness loop = EXECUTED flop of the current kernel, counted from the ncu
+# source page of a capture of the config1 shape (profiles/r1c_ga_invert_ncu.md: predicated-on thread instructions per
+# SASS opcode / lambda-points; FFMA2 = 4 flop, FMUL2 / FADD2 / FFMA = 2, FMUL / FADD = 1).  It is re-counted whenever the
+# kernel changes (r1a: 477, r1b: 280, r1c: 265.7), so `frac` is the FP32-pipe utilisation, not an inflated textbook
+# count.  See DESIGN.md "Measurement".  config0 (one line) is not the bench default and carries an estimate.
+FLOP_PER_POINT = {"config0_tiny": 150.0, "config1_map256": 265.7, "config3_fulldisc": 265.7}
+# DRAM traffic of ga_invert_kernel per pixel, from the same capture (dram__bytes_read.sum + write.sum) / pixels
+DRAM_BYTES_PER_PIXEL_NCU = 8.878848e6 / 4096
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 
 
@@ -39,6 +43,7 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-aux", action="store_true", help="skip the auxiliary me_synth (config2) measurement")
     return ap.parse_args()
 
 
@@ -189,6 +194,39 @@ def build_inputs(cfg, n_pixels, side, rank, torch, B):
     return ld, obs, mask_t, mu_t, n_active, truth
 
 
+def bench_me_synth(torch, B, peaks, P=1_000_000):
+    """BASELINE config 2: forward synthesis of P prior draws on the two-line 128-point grid, IQUV output + chi2 against
+    one fixed profile (and chi2 only, to separate ALU from the store stream).  Not the headline metric: reported beside it."""
+    c2 = W.config2(P)
+    lam, ld = c2["lam"], B.line_data_from_workload(c2["lines"], True)
+    L = int(lam.size)
+    params = torch.from_numpy(W.draw_truth(P, seed=W.SEED_TRUTH, stream=7).astype(np.float32)).cuda()
+    obs_ref, _ = B.me_synth(params[:1].contiguous(), lam, ld)
+    obs_ref = obs_ref[0].contiguous()
+    wos = c2["ga"]["stokes_weight"] / c2["ga"]["sigma"]
+    out = torch.empty((P, 4, L), dtype=torch.float32, device="cuda")
+    chi = torch.empty((P,), dtype=torch.float32, device="cuda")
+    res = {}
+    for name, kw in (("stokes_and_chi2", dict(out_stokes=out, out_chi2=chi)), ("chi2_only", dict(out_chi2=chi, want_stokes=False))):
+        for _ in range(3):
+            B.me_synth(params, lam, ld, obs_ref=obs_ref, w_over_sigma=wos, **kw)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 5
+        e0.record()
+        for _ in range(reps):
+            B.me_synth(params, lam, ld, obs_ref=obs_ref, w_over_sigma=wos, **kw)
+        e1.record()
+        torch.cuda.synchronize()
+        sec = e0.elapsed_time(e1) * 1e-3 / reps
+        nbytes = P * (36 + 4 + (16 * L if name == "stokes_and_chi2" else 0))
+        res[name] = {"syntheses_per_s": P / sec, "ms": sec * 1e3, "hbm_gbs": nbytes / sec / 1e9,
+                     "hbm_frac_of_measured": nbytes / sec / 1e9 / float(peaks.get("hbm_gbs", 6650.0))}
+    res["P"] = P
+    res["L"] = L
+    return res
+
+
 def run_b200(args):
     import torch
     from paper_1208_0302_b200 import binding as B, build as mebuild
@@ -285,6 +323,9 @@ def run_b200(args):
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     clocks = clk.summary()
+    # the FP32 FMA rate this box actually sustains (scalar FFMA probe of the library, 8 resident CTAs/SM), for context
+    from paper_1208_0302_b200 import peaks as mepeaks
+    probe = mepeaks.measure(iters=2048, kinds=(0, 3))["probes"]
     line = {"metric": "pixel-inversions/s", "value": value, "unit": "pixels/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -294,10 +335,15 @@ def run_b200(args):
                        "l2": "obs cube %.0f MB per step (> 126 MB L2 for config1/3); path is ALU-bound" % (obs.numel() * 4 / 1e6)},
             "syntheses_per_s": value * syn, "median_chi2": med_chi2,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": None, "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt,
+                         "traffic": DRAM_BYTES_PER_PIXEL_NCU * n_active, "algorithmic_bytes": (16 * L + 40) * n_active,
+                         "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt,
+                         "peak_measured_ffma_tflops": probe["ffma"]["tflops"],
+                         "mufu_per_s_measured": probe["mufu"]["thread_inst_per_s"],
                          "peak_basis": "148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (max SM clock)" % sm_max,
                          "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / sm_max)) if clocks.get("sm_mhz") else None},
             "clocks": clocks, "gpu_launches": args.steps, "e2e": e2e}
+    if not args.no_aux:
+        line["me_synth_config2"] = bench_me_synth(torch, B, peaks)
     if not args.no_cpu_baseline:
         from oracle import api as orc
         cores = orc.hardware_threads()

@@ -13,7 +13,7 @@ KINDS = {0: ("ffma", 1, 0, 0), 1: ("ffma2", 0, 1, 0), 2: ("ffma2+ffma 1:1", 1, 1
 FLOP_PER_SLOT = {0: 2.0, 1: 4.0, 2: 6.0, 3: 0.0, 4: 2.0, 5: 5.0, 6: 4.0, 7: 4.0, 8: 4.0, 9: 4.0, 10: 2.0}
 
 
-def measure(iters=4096, blocks_per_sm=8, repeats=5):
+def measure(iters=4096, blocks_per_sm=8, repeats=5, kinds=None):
     import torch
     from . import binding as B
     B.lib()
@@ -22,6 +22,8 @@ def measure(iters=4096, blocks_per_sm=8, repeats=5):
     scratch = torch.zeros(blocks * 256, dtype=torch.float32, device="cuda")
     out = {"sm_count": sms, "iters": iters, "blocks": blocks, "probes": {}}
     for kind, (name, n_ffma, n_ffma2, n_mufu) in KINDS.items():
+        if kinds is not None and kind not in kinds:
+            continue
         B.me_peak_probe(kind, 64, blocks, scratch)
         torch.cuda.synchronize()
         best = None

@@ -133,3 +133,37 @@ def test_config1_subset_full_parity(B):
     expect = 128 * 37.0 / (4 * 128 - 9)
     assert np.mean(gc.cpu().numpy() < 1.5 * expect) > 0.5
     print("config1 subset: identical-optimum fraction", frac)
+
+
+def test_config1_full_size_sampled_parity(B):
+    # BASELINE config 1 at FULL size (256 x 256 = 65 536 pixels, L = 128, pop 128, 100 generations), in the launch
+    # configuration bench.py times (one ga_invert call over the whole map).  The oracle cannot invert 65 536 pixels in
+    # test time, so (a) four blocks of 8 pixels (first, two interior, ragged last) are inverted by the oracle with the
+    # same global pixel ids and compared one by one, and (b) properties that hold at any size are checked on the map.
+    c1 = W.config1()
+    N = c1["n_pixels"]
+    truth, obs, ln = make_obs(c1, N, threads=NTHREADS)
+    ld = B.line_data_from_workload(c1["lines"], True)
+    gp, gc = B.ga_invert(dev(obs), c1["lam"], ld, c1["ga"], W.SEED_GA)
+    torch.cuda.synchronize()
+    gp, gc = gp.cpu().numpy().astype(np.float64), gc.cpu().numpy().astype(np.float64)
+    # (b) whole-map properties
+    assert np.all(np.isfinite(gc)) and np.all(np.isfinite(gp))
+    lo, hi = c1["ga"]["lo"], c1["ga"]["hi"]
+    assert np.all(gp >= lo * (1 - 1e-6) - 1e-6) and np.all(gp <= hi * (1 + 1e-6))
+    expect = 128 * 37.0 / (4 * 128 - 9)                       # E[chi2] at the truth (reading F11)
+    assert np.median(gc) < 1.6 * expect
+    assert np.mean(gc < 1.5 * expect) > 0.5
+    strong = truth[:, 0] > 1000.0                             # strong fields are well constrained at sigma = 1e-3
+    assert np.median(np.abs(gp[strong, 0] - truth[strong, 0]) / truth[strong, 0]) < 0.05
+    # (a) sampled pixels against the oracle, same Philox streams (keying by global pixel id)
+    same = []
+    for start in (0, 20000, 41234, N - 8):
+        sl = slice(start, start + 8)
+        res = orc.ga_invert(obs[sl], c1["lam"], ln, c1["ga"], seed=W.SEED_GA, pixel_base=start, threads=NTHREADS)
+        ok = np.abs(gc[sl] - res["chi2"]) <= 2e-4 * res["chi2"]
+        close = np.all(np.abs(gp[sl] - res["params"]) <= 1e-4 * (np.abs(res["params"]) + 1.0), axis=1)
+        same += list(ok & close)
+        # pixels that left the oracle's trajectory still land within the statistical tolerance
+        assert np.all(np.abs(gc[sl] - res["chi2"]) <= 0.25 * res["chi2"])
+    assert np.mean(same) >= 0.85, np.mean(same)
