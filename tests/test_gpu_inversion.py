@@ -61,7 +61,8 @@ def test_config0_tiny_full_parity(B):
     assert np.max(np.abs(gc.cpu().numpy() - chk) / chk) < 5e-4
     # parameters stay inside the box
     p = gp.cpu().numpy()
-    assert np.all(p >= c0["ga"]["lo"] * (1 - 1e-6) - 1e-6) and np.all(p <= c0["ga"]["hi"] * (1 + 1e-6))
+    lo, hi = c0["ga"]["lo"], c0["ga"]["hi"]
+    assert np.all(p >= lo - 1e-6 * np.abs(lo) - 1e-6) and np.all(p <= hi + 1e-6 * np.abs(hi) + 1e-6)
 
 
 def test_determinism_sharding_mask_and_mu(B):
@@ -150,7 +151,7 @@ def test_config1_full_size_sampled_parity(B):
     # (b) whole-map properties
     assert np.all(np.isfinite(gc)) and np.all(np.isfinite(gp))
     lo, hi = c1["ga"]["lo"], c1["ga"]["hi"]
-    assert np.all(gp >= lo * (1 - 1e-6) - 1e-6) and np.all(gp <= hi * (1 + 1e-6))
+    assert np.all(gp >= lo - 1e-6 * np.abs(lo) - 1e-6) and np.all(gp <= hi + 1e-6 * np.abs(hi) + 1e-6)
     expect = 128 * 37.0 / (4 * 128 - 9)                       # E[chi2] at the truth (reading F11)
     assert np.median(gc) < 1.6 * expect
     assert np.mean(gc < 1.5 * expect) > 0.5
