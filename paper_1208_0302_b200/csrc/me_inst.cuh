@@ -125,58 +125,86 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// me_synth: warp = parameter vector, lane = wavelength pair.  out_stokes[P,4,L]: each (vector, Stokes) row is
-// written as consecutive 128-byte warp stores.  chi2 (optional) is reduced with warp shuffles.
+// me_synth: thread = parameter vector (as in the GA kernel: the lanes of a warp sit at the SAME wavelength, so the
+// Voigt tier branches stay mostly warp-uniform), serial loop over wavelength pairs.  out_stokes[P,4,L] is written
+// through a warp-private shared-memory tile: every SYNTH_CW wavelengths the warp transposes its 32 vectors x 4 Stokes
+// rows and streams them out as 64-byte row segments (two per store instruction, full 32-byte sectors).
+// chi2 (optional) accumulates in registers as in the fused fitness.
+// Tile: [32 vectors][4 * SYNTH_CW + 1] floats per warp (odd stride: conflict-free on both sides).
 // ------------------------------------------------------------------------------------------------------------
+#define SYNTH_CW 16
+#define SYNTH_VS (4 * SYNTH_CW + 1)
+#define SYNTH_THREADS 128
+
 template <int NL, bool TRIPLET>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(SYNTH_THREADS, 4)
 me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
                 int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
                 float w2I, float w2Q, float w2U, float w2V, float inv_nu, float* __restrict__ out_chi2) {
-    const int lane = threadIdx.x & 31;
-    const int64_t warp0 = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    const int64_t nwarps = (int64_t)gridDim.x * (blockDim.x >> 5);
-    const int L = sd.L;
-    for (int64_t v = warp0; v < P; v += nwarps) {
+    extern __shared__ float4 smem4[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float* tile = reinterpret_cast<float*>(smem4) + warp * (32 * SYNTH_VS);
+    const int L = sd.L, npair = L >> 1;
+    const bool want_out = out_stokes != nullptr, want_chi2 = out_chi2 != nullptr;
+    for (int64_t base = (int64_t)blockIdx.x * SYNTH_THREADS; base < P; base += (int64_t)gridDim.x * SYNTH_THREADS) {
+        const int64_t wbase = base + warp * 32;                 // first vector of this warp
+        if (wbase >= P) continue;
+        const int64_t v = wbase + lane < P ? wbase + lane : P - 1;   // idle lanes recompute the last vector, never store
         float p[ME_NPAR];
 #pragma unroll
         for (int j = 0; j < ME_NPAR; ++j) p[j] = __ldg(params + v * ME_NPAR + j);
         const float mu = mu_arr != nullptr ? __ldg(mu_arr + v) : 1.0f;
         Individual<NL> ind;
         setup_individual<NL>(ind, p, mu, sd);
-        float acc = 0.f;
-        float* o = out_stokes != nullptr ? out_stokes + v * 4 * (int64_t)L : nullptr;
-        const bool even = (L & 1) == 0;                      // float2 rows are 8-byte aligned only for even L
-        for (int j = 2 * lane; j < L; j += 64) {
-            const bool tail = j + 1 >= L;
-            f2 I, Q, U, V;
-            stokes_pair<NL, TRIPLET>(ind, sd, j, tail, I, Q, U, V);
-            if (o != nullptr) {
-                if (even) {
-                    __stcs(reinterpret_cast<float2*>(o + j), I); __stcs(reinterpret_cast<float2*>(o + L + j), Q);
-                    __stcs(reinterpret_cast<float2*>(o + 2 * L + j), U); __stcs(reinterpret_cast<float2*>(o + 3 * L + j), V);
-                } else {
-                    __stcs(o + j, I.x); __stcs(o + L + j, Q.x); __stcs(o + 2 * L + j, U.x); __stcs(o + 3 * L + j, V.x);
-                    if (!tail) { __stcs(o + j + 1, I.y); __stcs(o + L + j + 1, Q.y); __stcs(o + 2 * L + j + 1, U.y); __stcs(o + 3 * L + j + 1, V.y); }
+        f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
+        for (int jp0 = 0; jp0 < npair; jp0 += SYNTH_CW / 2) {
+            const int nloc = min(SYNTH_CW / 2, npair - jp0);
+            for (int i = 0; i < nloc; ++i) {
+                const int j = 2 * (jp0 + i);
+                f2 I, Q, U, V;
+                stokes_pair<NL, TRIPLET>(ind, sd, j, false, I, Q, U, V);
+                if (want_out) {
+                    float* t = tile + lane * SYNTH_VS + 2 * i;
+                    t[0] = I.x; t[1] = I.y; t[SYNTH_CW] = Q.x; t[SYNTH_CW + 1] = Q.y;
+                    t[2 * SYNTH_CW] = U.x; t[2 * SYNTH_CW + 1] = U.y; t[3 * SYNTH_CW] = V.x; t[3 * SYNTH_CW + 1] = V.y;
+                }
+                if (want_chi2) {
+                    const f2 dI = sub2(make_float2(__ldg(obs_ref + j), __ldg(obs_ref + j + 1)), I);
+                    const f2 dQ = sub2(make_float2(__ldg(obs_ref + L + j), __ldg(obs_ref + L + j + 1)), Q);
+                    const f2 dU = sub2(make_float2(__ldg(obs_ref + 2 * L + j), __ldg(obs_ref + 2 * L + j + 1)), U);
+                    const f2 dV = sub2(make_float2(__ldg(obs_ref + 3 * L + j), __ldg(obs_ref + 3 * L + j + 1)), V);
+                    aI = fma2(dI, dI, aI); aQ = fma2(dQ, dQ, aQ); aU = fma2(dU, dU, aU); aV = fma2(dV, dV, aV);
                 }
             }
-            if (out_chi2 != nullptr) {
-                const float dI = __ldg(obs_ref + j) - I.x, dQ = __ldg(obs_ref + L + j) - Q.x;
-                const float dU = __ldg(obs_ref + 2 * L + j) - U.x, dV = __ldg(obs_ref + 3 * L + j) - V.x;
-                acc = fmaf(w2I * dI, dI, acc); acc = fmaf(w2Q * dQ, dQ, acc);
-                acc = fmaf(w2U * dU, dU, acc); acc = fmaf(w2V * dV, dV, acc);
-                if (!tail) {
-                    const float eI = __ldg(obs_ref + j + 1) - I.y, eQ = __ldg(obs_ref + L + j + 1) - Q.y;
-                    const float eU = __ldg(obs_ref + 2 * L + j + 1) - U.y, eV = __ldg(obs_ref + 3 * L + j + 1) - V.y;
-                    acc = fmaf(w2I * eI, eI, acc); acc = fmaf(w2Q * eQ, eQ, acc);
-                    acc = fmaf(w2U * eU, eU, acc); acc = fmaf(w2V * eV, eV, acc);
+            if (want_out) {
+                __syncwarp();
+                const int ncol = 2 * nloc, k = lane & 15;
+                const int64_t nvec = P - wbase < 32 ? P - wbase : 32;
+#pragma unroll 4
+                for (int it = 0; it < 64; ++it) {
+                    const int row = 2 * it + (lane >> 4), lv = row >> 2, st = row & 3;
+                    if (lv < nvec && k < ncol)
+                        __stcs(out_stokes + ((wbase + lv) * 4 + st) * (int64_t)L + 2 * jp0 + k, tile[lv * SYNTH_VS + st * SYNTH_CW + k]);
                 }
+                __syncwarp();
             }
         }
-        if (out_chi2 != nullptr) {
-#pragma unroll
-            for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
-            if (lane == 0) out_chi2[v] = acc * inv_nu;
+        if (L & 1) {                                             // odd tail: one wavelength, written directly
+            f2 I, Q, U, V;
+            stokes_pair<NL, TRIPLET>(ind, sd, L - 1, true, I, Q, U, V);
+            if (want_out && wbase + lane < P) {
+                float* o = out_stokes + v * 4 * (int64_t)L + (L - 1);
+                __stcs(o, I.x); __stcs(o + L, Q.x); __stcs(o + 2 * L, U.x); __stcs(o + 3 * L, V.x);
+            }
+            if (want_chi2) {
+                const float dI = __ldg(obs_ref + L - 1) - I.x, dQ = __ldg(obs_ref + 2 * L - 1) - Q.x;
+                const float dU = __ldg(obs_ref + 3 * L - 1) - U.x, dV = __ldg(obs_ref + 4 * L - 1) - V.x;
+                aI.x = fmaf(dI, dI, aI.x); aQ.x = fmaf(dQ, dQ, aQ.x); aU.x = fmaf(dU, dU, aU.x); aV.x = fmaf(dV, dV, aV.x);
+            }
+        }
+        if (want_chi2 && wbase + lane < P) {
+            const float sI = aI.x + aI.y, sQ = aQ.x + aQ.y, sU = aU.x + aU.y, sV = aV.x + aV.y;
+            out_chi2[v] = inv_nu * fmaf(w2I, sI, fmaf(w2Q, sQ, fmaf(w2U, sU, w2V * sV)));
         }
     }
 }
@@ -253,11 +281,12 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int64_t blocks_needed = (P + 7) / 8;                       // 8 warps per block
-    const int64_t cap = (int64_t)sms * 8;                            // persistent grid: 8 resident blocks per SM
+    const int64_t blocks_needed = (P + SYNTH_THREADS - 1) / SYNTH_THREADS;
+    const int64_t cap = (int64_t)sms * 4;                            // persistent grid: 4 resident blocks per SM
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
-    me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET><<<grid, 256, 0, st>>>(sd, params, mu, P, out_stokes, obs_ref, w2[0], w2[1],
-                                                                       w2[2], w2[3], inv_nu, out_chi2);
+    const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float);
+    me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET><<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, P, out_stokes, obs_ref, w2[0],
+                                                                                   w2[1], w2[2], w2[3], inv_nu, out_chi2);
     return cudaGetLastError();
 }
 

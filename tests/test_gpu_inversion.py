@@ -168,3 +168,34 @@ def test_config1_full_size_sampled_parity(B):
         # pixels that left the oracle's trajectory still land within the statistical tolerance
         assert np.all(np.abs(gc[sl] - res["chi2"]) <= 0.25 * res["chi2"])
     assert np.mean(same) >= 0.85, np.mean(same)
+
+
+def test_config3_fulldisc_shape_sampled_parity(B):
+    # BASELINE config 3 (full-disc mask, mu per pixel, 80 % quiet / 20 % active, B box [1, 3500] G, 200 generations)
+    # on a 64 x 64 rendition of the 2048 x 2048 map; launched as bench.py --workload config3 launches it (mask + mu).
+    # 16 active pixels (quiet and active-region) are inverted by the oracle with the same global ids.
+    c3 = W.config3(64)
+    mask, mu, truth, active = W.fulldisc_truth(c3["n_side"], c3["radius"])
+    N = mask.size
+    from helpers import oracle_lines
+    ln = oracle_lines(c3["lines"], True)
+    clean = orc.synth(truth, c3["lam"], ln, mu=mu, threads=NTHREADS)
+    obs = (clean + W.draw_noise(clean.shape, c3["sigma"])).astype(np.float32).astype(np.float64)
+    ld = B.line_data_from_workload(c3["lines"], True)
+    gp, gc = B.ga_invert(dev(obs), c3["lam"], ld, c3["ga"], W.SEED_GA, mask=dev(mask, np.uint8), mu=dev(mu))
+    torch.cuda.synchronize()
+    gp, gc = gp.cpu().numpy().astype(np.float64), gc.cpu().numpy().astype(np.float64)
+    on = mask.astype(bool)
+    assert abs(on.mean() - np.pi / 4 * (1000.0 / 1024.0) ** 2) < 0.02           # ~ pi/4 of the pixels are on the disc
+    assert np.isnan(gc[~on]).all() and np.isnan(gp[~on]).all() and np.isfinite(gc[on]).all()
+    # active-region pixels (B >= 500 G): field strength recovered
+    act = on & active
+    assert np.median(np.abs(gp[act, 0] - truth[act, 0]) / truth[act, 0]) < 0.05
+    # sampled pixels: 8 quiet + 8 active, oracle with mask/mu and the same pixel ids
+    idx = np.concatenate([np.flatnonzero(on & ~active)[::400][:8], np.flatnonzero(act)[::80][:8]])
+    same = []
+    for i in idx:
+        res = orc.ga_invert(obs[i:i + 1], c3["lam"], ln, c3["ga"], seed=W.SEED_GA, mu=mu[i:i + 1], pixel_base=int(i), threads=1)
+        same.append(abs(gc[i] - res["chi2"][0]) <= 2e-4 * res["chi2"][0])
+        assert abs(gc[i] - res["chi2"][0]) <= 0.25 * res["chi2"][0]
+    assert np.mean(same) >= 0.75, np.mean(same)
