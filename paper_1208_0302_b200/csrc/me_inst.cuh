@@ -130,10 +130,11 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 // through a warp-private shared-memory tile: every SYNTH_CW wavelengths the warp transposes its 32 vectors x 4 Stokes
 // rows and streams them out as 64-byte row segments (two per store instruction, full 32-byte sectors).
 // chi2 (optional) accumulates in registers as in the fused fitness.
-// Tile: [32 vectors][4 * SYNTH_CW + 1] floats per warp (odd stride: conflict-free on both sides).
+// Tile: [32 vectors][4 * SYNTH_CW + 4] floats per warp; rows are read back as float4 (8 rows = 512 B per store
+// instruction) when L % 4 == 0, else element-wise.
 // ------------------------------------------------------------------------------------------------------------
 #define SYNTH_CW 16
-#define SYNTH_VS (4 * SYNTH_CW + 1)
+#define SYNTH_VS (4 * SYNTH_CW + 4)      /* row stride: 16-byte aligned rows for LDS.128 / STG.128 */
 #define SYNTH_THREADS 128
 
 template <int NL, bool TRIPLET>
@@ -164,9 +165,8 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
                 f2 I, Q, U, V;
                 stokes_pair<NL, TRIPLET>(ind, sd, j, false, I, Q, U, V);
                 if (want_out) {
-                    float* t = tile + lane * SYNTH_VS + 2 * i;
-                    t[0] = I.x; t[1] = I.y; t[SYNTH_CW] = Q.x; t[SYNTH_CW + 1] = Q.y;
-                    t[2 * SYNTH_CW] = U.x; t[2 * SYNTH_CW + 1] = U.y; t[3 * SYNTH_CW] = V.x; t[3 * SYNTH_CW + 1] = V.y;
+                    float2* t = reinterpret_cast<float2*>(tile + lane * SYNTH_VS + 2 * i);
+                    t[0] = I; t[SYNTH_CW / 2] = Q; t[SYNTH_CW] = U; t[3 * SYNTH_CW / 2] = V;
                 }
                 if (want_chi2) {
                     const f2 dI = sub2(make_float2(__ldg(obs_ref + j), __ldg(obs_ref + j + 1)), I);
@@ -178,13 +178,25 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
             }
             if (want_out) {
                 __syncwarp();
-                const int ncol = 2 * nloc, k = lane & 15;
+                const int ncol = 2 * nloc;
                 const int64_t nvec = P - wbase < 32 ? P - wbase : 32;
+                if ((L & 3) == 0) {                                  // 16-byte aligned rows: 8 rows per store instruction
+                    const int q = 4 * (lane & 3);
 #pragma unroll 4
-                for (int it = 0; it < 64; ++it) {
-                    const int row = 2 * it + (lane >> 4), lv = row >> 2, st = row & 3;
-                    if (lv < nvec && k < ncol)
-                        __stcs(out_stokes + ((wbase + lv) * 4 + st) * (int64_t)L + 2 * jp0 + k, tile[lv * SYNTH_VS + st * SYNTH_CW + k]);
+                    for (int it = 0; it < 16; ++it) {
+                        const int row = 8 * it + (lane >> 2), lv = row >> 2, st = row & 3;
+                        if (lv < nvec && q < ncol)
+                            __stcs(reinterpret_cast<float4*>(out_stokes + ((wbase + lv) * 4 + st) * (int64_t)L + 2 * jp0 + q),
+                                   *reinterpret_cast<const float4*>(tile + lv * SYNTH_VS + st * SYNTH_CW + q));
+                    }
+                } else {
+                    const int k = lane & 15;
+#pragma unroll 4
+                    for (int it = 0; it < 64; ++it) {
+                        const int row = 2 * it + (lane >> 4), lv = row >> 2, st = row & 3;
+                        if (lv < nvec && k < ncol)
+                            __stcs(out_stokes + ((wbase + lv) * 4 + st) * (int64_t)L + 2 * jp0 + k, tile[lv * SYNTH_VS + st * SYNTH_CW + k]);
+                    }
                 }
                 __syncwarp();
             }
