@@ -85,13 +85,31 @@ class Lines:
                 _p(self.shift, C.c_double), _p(self.weight, C.c_double), _p(self.kind, C.c_int), C.c_double(self.lambda_ref)]
 
 
-def synth(params, lam, lines, mu=None, use_solve=False, threads=1):
-    params = _f64(params).reshape(-1, NPAR)
+def _npar(cfg):
+    return int(len(cfg["lo"]))
+
+
+def _nm(nm_profile, npar, L):
+    if npar == NPAR:
+        return None
+    assert npar == 11 and nm_profile is not None, "the 11-parameter model needs nm_profile[L] (reading F13)"
+    a = _f64(nm_profile)
+    assert a.shape == (L,)
+    return a
+
+
+def synth(params, lam, lines, mu=None, use_solve=False, threads=1, nm_profile=None):
+    """params[P,9], or [P,11] with nm_profile[L] (11-parameter model, reading F13)."""
+    params = _f64(params)
+    npar = params.shape[-1] if params.ndim > 1 else params.size
+    assert npar in (9, 11)
+    params = params.reshape(-1, npar)
     lam = _f64(lam)
     P, L = params.shape[0], lam.size
     mu_a = _f64(mu) if mu is not None else None
+    nm = _nm(nm_profile, npar, L)
     out = np.empty((P, 4, L))
-    lib().orc_synth(_p(params, C.c_double), _p(mu_a, C.c_double), C.c_int64(P), _p(lam, C.c_double), C.c_int(L),
+    lib().orc_synth(_p(params, C.c_double), C.c_int(npar), _p(nm, C.c_double), _p(mu_a, C.c_double), C.c_int64(P), _p(lam, C.c_double), C.c_int(L),
                     *lines.args(), C.c_int(int(use_solve)), C.c_int(threads), _p(out, C.c_double))
     return out
 
@@ -124,16 +142,17 @@ def philox_raw(ctr, key):
 
 
 def decode(genes, cfg):
-    genes = np.ascontiguousarray(genes, dtype=np.float32).reshape(-1, NPAR)
+    npar = _npar(cfg)
+    genes = np.ascontiguousarray(genes, dtype=np.float32).reshape(-1, npar)
     out = np.empty(genes.shape)
     lo, hi, lg = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"])
-    lib().orc_decode(_p(genes, C.c_float), C.c_int64(genes.shape[0]), _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(out, C.c_double))
+    lib().orc_decode(_p(genes, C.c_float), C.c_int(npar), C.c_int64(genes.shape[0]), _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(out, C.c_double))
     return out
 
 
-def ga_init(N, pop, seed, pixel_base=0):
-    genes = np.empty((N, pop, NPAR), dtype=np.float32)
-    lib().orc_ga_init(C.c_int64(N), C.c_uint64(pixel_base), C.c_int(pop), C.c_uint64(seed), _p(genes, C.c_float))
+def ga_init(N, pop, seed, pixel_base=0, npar=NPAR):
+    genes = np.empty((N, pop, npar), dtype=np.float32)
+    lib().orc_ga_init(C.c_int64(N), C.c_uint64(pixel_base), C.c_int(pop), C.c_int(npar), C.c_uint64(seed), _p(genes, C.c_float))
     return genes
 
 
@@ -153,27 +172,30 @@ def ga_step(genes, chi2v, t, cfg, seed, pixel_base=0):
     keep, a = _cfg_args(cfg)
     per = _i32(cfg["periodic"])
     lib().orc_ga_step(_p(genes, C.c_float), _p(chi2v, C.c_double), C.c_int64(N), C.c_uint64(pixel_base), C.c_int(t),
-                      *a, _p(per, C.c_int), C.c_uint64(seed), _p(out, C.c_float))
+                      *a, _p(per, C.c_int), C.c_int(genes.shape[2]), C.c_uint64(seed), _p(out, C.c_float))
     return out
 
 
-def ga_fitness(genes, obs, lam, lines, cfg, mu=None, threads=1):
+def ga_fitness(genes, obs, lam, lines, cfg, mu=None, threads=1, nm_profile=None):
     genes = np.ascontiguousarray(genes, dtype=np.float32)
     N, pop = genes.shape[0], genes.shape[1]
     obs, lam = _f64(obs), _f64(lam)
     mu_a = _f64(mu) if mu is not None else None
     lo, hi, lg = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"])
     w, sg = _f64(cfg["stokes_weight"]), _f64(cfg["sigma"])
+    npar = _npar(cfg)
+    assert genes.shape[2] == npar
+    nm = _nm(nm_profile, npar, lam.size)
     out = np.empty((N, pop))
     lib().orc_ga_fitness(_p(genes, C.c_float), _p(obs, C.c_double), _p(mu_a, C.c_double), C.c_int64(N), C.c_int(pop),
                          _p(lam, C.c_double), C.c_int(lam.size), *lines.args(),
                          _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(w, C.c_double), _p(sg, C.c_double),
-                         C.c_int(threads), _p(out, C.c_double))
+                         C.c_int(npar), _p(nm, C.c_double), C.c_int(threads), _p(out, C.c_double))
     return out
 
 
-def ga_invert(obs, lam, lines, cfg, seed, mask=None, mu=None, pixel_base=0, threads=1, want_trace=False):
-    """obs[N,4,L] -> dict(params[N,9], chi2[N], genes[N,9], trace[N,G+1] or None)."""
+def ga_invert(obs, lam, lines, cfg, seed, mask=None, mu=None, pixel_base=0, threads=1, want_trace=False, nm_profile=None):
+    """obs[N,4,L] -> dict(params[N,M], chi2[N], genes[N,M], trace[N,G+1] or None); M = len(cfg["lo"]) = 9 or 11."""
     obs, lam = _f64(obs), _f64(lam)
     N, L = obs.shape[0], lam.size
     assert obs.shape == (N, 4, L)
@@ -182,12 +204,14 @@ def ga_invert(obs, lam, lines, cfg, seed, mask=None, mu=None, pixel_base=0, thre
     lo, hi, lg, per = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"]), _i32(cfg["periodic"])
     w, sg = _f64(cfg["stokes_weight"]), _f64(cfg["sigma"])
     keep, a = _cfg_args(cfg)
-    params, chi2v = np.empty((N, NPAR)), np.empty(N)
-    genes = np.full((N, NPAR), np.nan, dtype=np.float32)
+    npar = _npar(cfg)
+    nm = _nm(nm_profile, npar, L)
+    params, chi2v = np.empty((N, npar)), np.empty(N)
+    genes = np.full((N, npar), np.nan, dtype=np.float32)
     trace = np.full((N, cfg["generations"] + 1), np.nan) if want_trace else None
     lib().orc_ga_invert(_p(obs, C.c_double), _p(mask_a, C.c_ubyte), _p(mu_a, C.c_double), C.c_int64(N), C.c_uint64(pixel_base),
                         _p(lam, C.c_double), C.c_int(L), *lines.args(), *a,
                         _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(per, C.c_int),
-                        _p(w, C.c_double), _p(sg, C.c_double), C.c_uint64(seed), C.c_int(threads),
+                        _p(w, C.c_double), _p(sg, C.c_double), C.c_int(npar), _p(nm, C.c_double), C.c_uint64(seed), C.c_int(threads),
                         _p(params, C.c_double), _p(chi2v, C.c_double), _p(genes, C.c_float), _p(trace, C.c_double))
     return {"params": params, "chi2": chi2v, "genes": genes, "trace": trace}

@@ -34,10 +34,10 @@ double decode_gene(float g, double lo, double hi, int log_scale) {
 // G2: generation 0, gene j of individual i = lane (j mod 4) of block floor(j / 4).
 void ga_init(uint64_t pixel, const GaCfg& c, float* genes) {
     for (int i = 0; i < c.pop; ++i)
-        for (int j = 0; j < NPAR; ++j) {
+        for (int j = 0; j < c.npar; ++j) {
             uint32_t r[4];
             draw(c, pixel, 0, i, j / 4, r);
-            genes[i * NPAR + j] = u01(r[j % 4]);
+            genes[i * c.npar + j] = u01(r[j % 4]);
         }
 }
 
@@ -58,8 +58,9 @@ static int tournament(const uint32_t r[4], const double* chi2v, const GaCfg& c) 
 }
 
 void ga_step(const float* genes, const double* chi2v, int t, uint64_t pixel, const GaCfg& c, float* out) {
+    const int M = c.npar;
     const int elite = argmin(chi2v, c.pop);
-    for (int j = 0; j < NPAR; ++j) out[j] = genes[elite * NPAR + j];         // slot 0 <- elite of t-1
+    for (int j = 0; j < M; ++j) out[j] = genes[elite * M + j];               // slot 0 <- elite of t-1
     const float s_t = c.mut_scale[t];
     for (int i = 1; i < c.pop; ++i) {
         uint32_t r[4];
@@ -68,8 +69,8 @@ void ga_step(const float* genes, const double* chi2v, int t, uint64_t pixel, con
         draw(c, pixel, t, i, 2, r);
         const bool cross = u01(r[0]) < c.p_cross;
         const float alpha = u01(r[1]);
-        for (int j = 0; j < NPAR; ++j) {
-            const float gA = genes[A * NPAR + j], gB = genes[B * NPAR + j];
+        for (int j = 0; j < M; ++j) {
+            const float gA = genes[A * M + j], gB = genes[B * M + j];
             float g = gA;
             if (cross) { const float d = gA - gB; g = std::fmaf(alpha, d, gB); }    // arithmetic crossover
             if (j % 2 == 0) draw(c, pixel, t, i, 3 + j / 2, r);                     // pair (u_2j, u_2j+1)
@@ -77,40 +78,41 @@ void ga_step(const float* genes, const double* chi2v, int t, uint64_t pixel, con
             if (um < c.p_mut) { const float step = 2.0f * ud - 1.0f; g = std::fmaf(s_t, step, g); }
             if (c.periodic[j]) g = g - std::floor(g);                               // wrap (azimuth)
             else g = std::fmin(std::fmax(g, 0.0f), 1.0f);                           // clamp to the box (eq. 4)
-            out[i * NPAR + j] = g;
+            out[i * M + j] = g;
         }
     }
 }
 
 static double fitness(const float* g, const double* obs, double mu, const double* lambda, int L,
                       const Lines& ln, const GaCfg& c, std::vector<double>& model) {
-    double p[NPAR];
-    for (int j = 0; j < NPAR; ++j) p[j] = decode_gene(g[j], c.lo[j], c.hi[j], c.log_scale[j]);
-    synth(p, mu, lambda, L, ln, model.data(), false);
-    double x = chi2(obs, model.data(), L, c.w, c.sigma, NPAR);
+    double p[MAXPAR];
+    for (int j = 0; j < c.npar; ++j) p[j] = decode_gene(g[j], c.lo[j], c.hi[j], c.log_scale[j]);
+    synth_n(p, c.npar, mu, lambda, L, ln, c.nm_profile, model.data(), false);
+    double x = chi2(obs, model.data(), L, c.w, c.sigma, c.npar);                     // nu = 4L - M
     if (!std::isfinite(x)) x = std::numeric_limits<double>::infinity();              // G4
     return x;
 }
 
 void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c,
                      uint64_t pixel, double* best_params, double* best_chi2, float* best_genes, double* trace) {
-    std::vector<float> genes(c.pop * NPAR), next(c.pop * NPAR);
+    const int M = c.npar;
+    std::vector<float> genes(c.pop * M), next(c.pop * M);
     std::vector<double> f(c.pop), fnext(c.pop), model(4 * L);
     ga_init(pixel, c, genes.data());
-    for (int i = 0; i < c.pop; ++i) f[i] = fitness(&genes[i * NPAR], obs, mu, lambda, L, ln, c, model);
+    for (int i = 0; i < c.pop; ++i) f[i] = fitness(&genes[i * M], obs, mu, lambda, L, ln, c, model);
     if (trace) trace[0] = f[argmin(f.data(), c.pop)];
     for (int t = 1; t <= c.generations; ++t) {
         const int elite = argmin(f.data(), c.pop);
         ga_step(genes.data(), f.data(), t, pixel, c, next.data());
         fnext[0] = f[elite];                                                          // carried, not re-evaluated
-        for (int i = 1; i < c.pop; ++i) fnext[i] = fitness(&next[i * NPAR], obs, mu, lambda, L, ln, c, model);
+        for (int i = 1; i < c.pop; ++i) fnext[i] = fitness(&next[i * M], obs, mu, lambda, L, ln, c, model);
         genes.swap(next); f.swap(fnext);
         if (trace) trace[t] = f[argmin(f.data(), c.pop)];
     }
     const int b = argmin(f.data(), c.pop);                                             // G5
-    for (int j = 0; j < NPAR; ++j) {
-        best_params[j] = decode_gene(genes[b * NPAR + j], c.lo[j], c.hi[j], c.log_scale[j]);
-        if (best_genes) best_genes[j] = genes[b * NPAR + j];
+    for (int j = 0; j < M; ++j) {
+        best_params[j] = decode_gene(genes[b * M + j], c.lo[j], c.hi[j], c.log_scale[j]);
+        if (best_genes) best_genes[j] = genes[b * M + j];
     }
     *best_chi2 = f[b];
 }

@@ -16,6 +16,8 @@
 //   synth          pinned  (B=0 and gamma=0 closed forms, 4x4 solve of eq. 12, symmetries, weak field)
 //   chi2           pinned  (expected value at truth, brute-force grid minimum)
 //   philox4x32_10  pinned  (published known-answer vectors of Salmon et al. 2011)
+//   synth_n (11 parameters, reading F13) pinned (alpha=1,s=0 -> synth; alpha=0 -> B=0 closed form; s=1 -> I_fixed;
+//                  Q,U,V scale with (1-s) alpha; bilinearity in alpha and s)
 //   ga             operators pinned by brute-force re-derivation in Python on tiny inputs and by
 //                  invariants; absolute recovery accuracy: PARITY UNPINNED (the paper prints no
 //                  reproducible recovery numbers, Table 4 PAPER.md:340-345 is for SOLIS data).
@@ -44,7 +46,11 @@ struct Lines { std::vector<Line> lines; double lambda_ref; };
 
 // Parameter order (BASELINE config 0; differs from eq. 14):
 // [B (G), gamma (deg), chi (deg), eta0, dlambdaD (mA at lambda_ref), a, v_los (km/s), S0, S1]
-enum { P_B = 0, P_GAMMA, P_CHI, P_ETA0, P_DLD, P_A, P_VLOS, P_S0, P_S1, NPAR = 9 };
+enum { P_B = 0, P_GAMMA, P_CHI, P_ETA0, P_DLD, P_A, P_VLOS, P_S0, P_S1, NPAR = 9,
+       P_ALPHA = 9, P_STRAY = 10, MAXPAR = 11 };
+// 11-parameter model (eq. 19 PAPER.md:245-247 + stray light PAPER.md:251; reading F13 of DESIGN.md):
+//   I = (1 - s) [ alpha I^M(p) + (1 - alpha) I(p; B = 0) e ] + s I_fixed(lambda) e
+// alpha = magnetic fill fraction, s = stray-light fraction, I_fixed = a fixed unpolarised profile (nm_profile[L]).
 
 // Absorption-matrix elements at one wavelength (eq. 8; reading F1/F2).
 struct Eta { double eI, eQ, eU, eV, rQ, rU, rV; };
@@ -57,6 +63,9 @@ void stokes_by_solve(const Eta& e, double S0, double muS1, double out[4]);
 
 // Full profile: out[4][L].  use_solve selects the second path.
 void synth(const double* p, double mu, const double* lambda, int L, const Lines& ln, double* out, bool use_solve);
+// The same for npar = 9 (identical to synth) or npar = 11 (reading F13; nm_profile[L] is I_fixed).
+void synth_n(const double* p, int npar, double mu, const double* lambda, int L, const Lines& ln,
+             const double* nm_profile, double* out, bool use_solve);
 
 // eq. 16, reading F11: chi2 = 1/nu * sum_s sum_j (w_s/sigma_s)^2 (O - M)^2, nu = 4L - M.
 double chi2(const double* obs, const double* model, int L, const double w[4], const double sigma[4], int M);
@@ -69,8 +78,10 @@ struct GaCfg {
     int pop, generations, tournament_k;
     float p_cross, p_mut;
     std::vector<float> mut_scale;              // s_t for t = 0..generations (built by the caller, binary32)
-    double lo[NPAR], hi[NPAR];
-    int log_scale[NPAR], periodic[NPAR];
+    int npar = NPAR;                           // 9 or 11 genes
+    const double* nm_profile = nullptr;        // I_fixed[L] for npar = 11
+    double lo[MAXPAR], hi[MAXPAR];
+    int log_scale[MAXPAR], periodic[MAXPAR];
     double w[4], sigma[4];
     uint64_t seed;
 };

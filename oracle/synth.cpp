@@ -4,6 +4,7 @@
 // F1-F12), which restates eq. 7-16 of the paper.
 #include "oracle.hpp"
 #include <cmath>
+#include <vector>
 
 namespace orc {
 
@@ -87,6 +88,27 @@ void synth(const double* p, double mu, const double* lambda, int L, const Lines&
         if (use_solve) stokes_by_solve(e, p[P_S0], mu * p[P_S1], s);
         else stokes_closed_form(e, p[P_S0], mu * p[P_S1], s);
         for (int k = 0; k < 4; ++k) out[k * L + j] = s[k];
+    }
+}
+
+// 11-parameter model, reading F13: eq. 19 mixes the magnetic profile with a non-magnetic
+// one by the fill fraction alpha; the non-magnetic component is the SAME atmosphere with B = 0; a fraction s of stray
+// light with a fixed unpolarised profile is added on top (PAPER.md:251 treats it as a fixed 5 % correction; BASELINE
+// config 4 makes it a free parameter):
+//   I = (1 - s) [ alpha I^M(p) + (1 - alpha) I(p; B = 0) e ] + s I_fixed e.
+void synth_n(const double* p, int npar, double mu, const double* lambda, int L, const Lines& ln,
+             const double* nm_profile, double* out, bool use_solve) {
+    synth(p, mu, lambda, L, ln, out, use_solve);                 // I^M(p): the first nine parameters
+    if (npar == NPAR) return;
+    const double alpha = p[P_ALPHA], s = p[P_STRAY];
+    double q[NPAR];
+    for (int j = 0; j < NPAR; ++j) q[j] = p[j];
+    q[P_B] = 0.0;                                                // the same atmosphere without field
+    std::vector<double> nm(4 * L);
+    synth(q, mu, lambda, L, ln, nm.data(), use_solve);
+    for (int j = 0; j < L; ++j) {
+        out[j] = (1.0 - s) * (alpha * out[j] + (1.0 - alpha) * nm[j]) + s * nm_profile[j];
+        for (int k = 1; k < 4; ++k) out[k * L + j] = (1.0 - s) * alpha * out[k * L + j];   // e = (1,0,0,0)
     }
 }
 

@@ -24,12 +24,18 @@ def grid(centre, L, step):
     return centre + (np.arange(L, dtype=np.float64) - 0.5 * (L - 1)) * step
 
 
-def prior_box(b_lo=10.0, b_hi=3000.0):
+# 11-parameter model (reading F13): genes 9, 10 = magnetic fill fraction alpha in [0,1], stray-light fraction s in [0,0.3].
+# The fixed unpolarised profile I_fixed is the B = 0 profile of this parameter vector at mu = 1 (a typical quiet-Sun
+# atmosphere); whichever side consumes it synthesises it (this module holds no arithmetic of the method).
+NM_PARAMS = np.array([0.0, 0.0, 0.0, 12.0, 30.0, 0.2, 0.0, 0.25, 0.75])
+
+
+def prior_box(b_lo=10.0, b_hi=3000.0, npar=NPAR):
     """GA search box = the config's prior box (reading G1)."""
-    lo = np.array([b_lo, 0.0, 0.0, 1.0, 20.0, 0.01, -3.0, 0.1, 0.5])
-    hi = np.array([b_hi, 180.0, 180.0, 50.0, 45.0, 0.5, 3.0, 0.4, 1.0])
-    log_scale = np.array([1, 0, 0, 0, 0, 0, 0, 0, 0], dtype=np.int32)
-    periodic = np.array([0, 0, 1, 0, 0, 0, 0, 0, 0], dtype=np.int32)
+    lo = np.array([b_lo, 0.0, 0.0, 1.0, 20.0, 0.01, -3.0, 0.1, 0.5, 0.0, 0.0])[:npar]
+    hi = np.array([b_hi, 180.0, 180.0, 50.0, 45.0, 0.5, 3.0, 0.4, 1.0, 1.0, 0.3])[:npar]
+    log_scale = np.array([1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0], dtype=np.int32)[:npar]
+    periodic = np.array([0, 0, 1, 0, 0, 0, 0, 0, 0, 0, 0], dtype=np.int32)[:npar]
     return lo, hi, log_scale, periodic
 
 
@@ -40,19 +46,24 @@ def mutation_schedule(generations, s0=0.5, s_end=0.0025):
 
 
 def ga_config(pop, generations, sigma=1e-3, b_lo=10.0, b_hi=3000.0, tournament_k=3, p_cross=0.8, p_mut=None,
-              s0=0.5, s_end=0.0025, stokes_weight=(1.0, 4.0, 4.0, 2.0)):
-    lo, hi, log_scale, periodic = prior_box(b_lo, b_hi)
+              s0=0.5, s_end=0.0025, stokes_weight=(1.0, 4.0, 4.0, 2.0), npar=NPAR):
+    lo, hi, log_scale, periodic = prior_box(b_lo, b_hi, npar)
     return dict(pop=int(pop), generations=int(generations), tournament_k=int(tournament_k),
-                p_cross=float(np.float32(p_cross)), p_mut=float(np.float32(2.0 / NPAR if p_mut is None else p_mut)),
+                p_cross=float(np.float32(p_cross)), p_mut=float(np.float32(2.0 / npar if p_mut is None else p_mut)),
                 mut_scale=mutation_schedule(generations, s0, s_end), lo=lo, hi=hi, log_scale=log_scale, periodic=periodic,
                 stokes_weight=np.asarray(stokes_weight, dtype=np.float64), sigma=np.full(4, float(sigma)))
 
 
-def draw_truth(n, seed=SEED_TRUTH, b_lo=10.0, b_hi=3000.0, stream=0):
-    """iid prior draws (BASELINE config 0): B log-uniform, the rest uniform, S1 = 1 - S0."""
+def draw_truth(n, seed=SEED_TRUTH, b_lo=10.0, b_hi=3000.0, stream=0, npar=NPAR):
+    """iid prior draws (BASELINE config 0): B log-uniform, the rest uniform, S1 = 1 - S0;
+    npar = 11 (config 4) appends alpha U[0,1] and s U[0,0.3] from a separate stream."""
     rng = np.random.Generator(np.random.Philox(key=[seed, stream]))
     u = rng.random((n, NPAR))
-    p = np.empty((n, NPAR))
+    p = np.empty((n, npar))
+    if npar == 11:
+        u2 = np.random.Generator(np.random.Philox(key=[seed, 1000 + stream])).random((n, 2))
+        p[:, 9] = u2[:, 0]
+        p[:, 10] = 0.3 * u2[:, 1]
     p[:, 0] = b_lo * (b_hi / b_lo) ** u[:, 0]
     p[:, 1] = 180.0 * u[:, 1]
     p[:, 2] = 180.0 * u[:, 2]
@@ -86,6 +97,14 @@ def config2(P=1_000_000):
     c = config1()
     c.update(name="config2_synth_sweep", n_pixels=P)
     return c
+
+
+def config4(n_side=512):
+    """Stress: 512x512, 11-parameter ME (reading F13), two-line 256-point grid at 12 mA, B log-U[1,500], sigma 3e-3,
+    pop 512, 300 generations."""
+    return dict(name="config4_stress11", n_pixels=n_side * n_side, lines=[FE_6301, FE_6302], triplets=True,
+                lam=grid(6302.0, 256, 0.012), ga=ga_config(512, 300, sigma=3e-3, b_lo=1.0, b_hi=500.0, npar=11),
+                sigma=3e-3, b_range=(1.0, 500.0), npar=11)
 
 
 def config3(n_side=2048, radius=1000.0):
