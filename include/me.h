@@ -34,7 +34,8 @@
 extern "C" {
 #endif
 
-#define ME_NPAR        9      /* model parameters / genes per individual */
+#define ME_NPAR        9      /* model parameters / genes per individual (base model, eq. 14) */
+#define ME_MAX_NPAR    11     /* with fill fraction alpha [9] and stray-light fraction s [10] (n_params = 11) */
 #define ME_MAX_LINES   4
 #define ME_MAX_COMP    48     /* Zeeman components summed over all lines */
 #define ME_MAX_L       512    /* wavelength samples */
@@ -46,7 +47,7 @@ typedef enum {
     ME_ERR_NULL = -1,         /* a required pointer is NULL */
     ME_ERR_SHAPE = -2,        /* a size is out of range (L, P, N, pop, n_lines, n_comp ...) */
     ME_ERR_RANGE = -3,        /* a value is out of range (lo > hi, sigma <= 0, log-scaled gene with lo <= 0 ...) */
-    ME_ERR_UNSUPPORTED = -4,  /* valid request that this build does not implement (n_params = 11) */
+    ME_ERR_UNSUPPORTED = -4,  /* valid request that this build does not implement (elite != 1) */
     ME_ERR_CUDA = -5          /* a CUDA runtime call failed; see me_last_cuda_error() */
 } me_status;
 
@@ -64,15 +65,18 @@ typedef struct {
     int n_lines;              /* 1..ME_MAX_LINES */
     const me_line* lines;     /* host [n_lines] */
     double lambda_ref_A;      /* wavelength at which dlambdaD is quoted; dlambdaD_l = dlambdaD * lambda_l / lambda_ref */
-    int n_params;             /* 9 (11 = fill fraction + stray light: ME_ERR_UNSUPPORTED in this build) */
-    const float* nm_profile;  /* reserved for n_params = 11; must be NULL */
+    int n_params;             /* 9, or 11: adds [9] alpha = magnetic fill fraction (eq. 19) and
+                                 [10] s = stray-light fraction:
+                                   I = (1-s) [ alpha I^M(p) + (1-alpha) I(p; B=0) e ] + s I_fixed e   (reading F13) */
+    const float* nm_profile;  /* DEVICE [L] f32: I_fixed, the fixed unpolarised profile; required for n_params = 11,
+                                 must be NULL for n_params = 9 */
 } me_line_data;
 
 /* ME forward synthesis (eq. 12-13, 15) of P parameter vectors on an L-point grid.
- *   params        device [P, 9] f32          mu          device [P] f32 or NULL (=> 1)
+ *   params        device [P, n_params] f32   mu          device [P] f32 or NULL (=> 1)
  *   lambda_grid_A host [L] f64 (Angstrom)    out_stokes  device [P, 4, L] f32 or NULL
  *   obs_ref       device [4, L] f32 or NULL  w_over_sigma host [4] f32 (w_s / sigma_s of eq. 16) or NULL
- *   out_chi2      device [P] f32 or NULL: chi2 of each vector against obs_ref, nu = 4L - 9.
+ *   out_chi2      device [P] f32 or NULL: chi2 of each vector against obs_ref, nu = 4L - n_params.
  * At least one of out_stokes / out_chi2 must be given; out_chi2 requires obs_ref and w_over_sigma. P = 0 is a no-op. */
 int me_synth(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
              const me_line_data* line_data, float* out_stokes,
@@ -89,9 +93,10 @@ typedef struct {
     float mut_scale0;         /* mutation half-width at t = 0 and t = G, geometric in between:            */
     float mut_scale_end;      /*   s_t = s0 (s_end/s0)^(t/G), built on the host in double, rounded to f32 */
     const float* mut_scale_table; /* host [generations+1] or NULL; if given it replaces the schedule above */
-    float lo[ME_NPAR], hi[ME_NPAR];  /* per-gene box (eq. 4); lo == hi fixes a gene */
-    uint8_t log_scale[ME_NPAR];      /* decode p = lo (hi/lo)^g instead of lo + (hi-lo) g */
-    uint8_t periodic[ME_NPAR];       /* gene wraps (g - floor g) instead of clamping to [0,1] */
+    float lo[ME_MAX_NPAR], hi[ME_MAX_NPAR];  /* per-gene box (eq. 4); lo == hi fixes a gene; the first
+                                                n_params entries are used */
+    uint8_t log_scale[ME_MAX_NPAR];  /* decode p = lo (hi/lo)^g instead of lo + (hi-lo) g */
+    uint8_t periodic[ME_MAX_NPAR];   /* gene wraps (g - floor g) instead of clamping to [0,1] */
     float stokes_weight[4];   /* w_s of eq. 16 (1,4,4,2 in the configs); enters squared */
     const float* mu;          /* device [N] f32 or NULL (=> 1): cosine of the heliocentric angle per pixel */
     int64_t pixel_id_base;    /* added to the pixel index in the RNG key so that shards reproduce the full run */
@@ -100,7 +105,7 @@ typedef struct {
 /* GA inversion of N pixels.
  *   obs    device [N, 4, L] f32            mask   device [N] u8 or NULL; 0 => pixel skipped, outputs NaN
  *   sigma  host [4] f32 per-Stokes noise   seed   Philox key
- *   out_params device [N, 9] f32 (decoded best individual)   out_chi2 device [N] f32 (its chi2, eq. 16)
+ *   out_params device [N, n_params] f32 (decoded best individual)   out_chi2 device [N] f32 (its chi2, eq. 16)
  * RNG: Philox4x32-10, key = (seed lo, seed hi), counter = (pixel_id_base + n, generation, individual, block).
  * Requires pixel_id_base + N <= 2^32. N = 0 is a no-op. */
 int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sigma,
@@ -109,14 +114,14 @@ int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sig
 
 /* Test hooks (not timed). */
 /* One generation t >= 1 of selection/crossover/mutation/elitism from given genes and given fitness. */
-int ga_step(const float* genes_in /*[N,pop,9]*/, const float* chi2_in /*[N,pop]*/, int64_t N, int generation,
-            const ga_cfg* cfg, int n_params, uint64_t seed, float* genes_out /*[N,pop,9]*/, void* stream);
+int ga_step(const float* genes_in /*[N,pop,n_params]*/, const float* chi2_in /*[N,pop]*/, int64_t N, int generation,
+            const ga_cfg* cfg, int n_params, uint64_t seed, float* genes_out /*[N,pop,n_params]*/, void* stream);
 /* The fused fitness alone: decode -> synthesis -> chi2 for every individual of every pixel. */
-int ga_fitness(const float* genes /*[N,pop,9]*/, const float* obs /*[N,4,L]*/, int64_t N, const float* sigma /*host[4]*/,
+int ga_fitness(const float* genes /*[N,pop,n_params]*/, const float* obs /*[N,4,L]*/, int64_t N, const float* sigma /*host[4]*/,
                const double* lambda_grid_A, int L, const me_line_data* line_data, const ga_cfg* cfg,
                float* chi2_out /*[N,pop]*/, void* stream);
-/* Generation-0 population (reading G2): genes_out device [N,pop,9]. */
-int ga_init(int64_t N, const ga_cfg* cfg, uint64_t seed, float* genes_out, void* stream);
+/* Generation-0 population (reading G2): genes_out device [N,pop,n_params]. */
+int ga_init(int64_t N, const ga_cfg* cfg, int n_params, uint64_t seed, float* genes_out, void* stream);
 /* One Philox4x32-10 block computed ON THE DEVICE; out is a HOST pointer; synchronises. */
 int me_philox(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t out[4]);
 /* n blocks with counters (c0_base + i, c1, c2, c3): out device [n,4] u32. */

@@ -10,6 +10,7 @@ import os
 import numpy as np
 
 NPAR = 9
+MAX_NPAR = 11      # with fill fraction and stray-light fraction (include/me.h ME_MAX_NPAR)
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libme_b200.so")
 _lib = None
@@ -42,8 +43,8 @@ class _GaCfg(C.Structure):
     _fields_ = [("pop", C.c_int), ("generations", C.c_int), ("tournament_k", C.c_int), ("elite", C.c_int),
                 ("p_cross", C.c_float), ("p_mut", C.c_float), ("mut_scale0", C.c_float), ("mut_scale_end", C.c_float),
                 ("mut_scale_table", C.POINTER(C.c_float)),
-                ("lo", C.c_float * NPAR), ("hi", C.c_float * NPAR),
-                ("log_scale", C.c_uint8 * NPAR), ("periodic", C.c_uint8 * NPAR),
+                ("lo", C.c_float * MAX_NPAR), ("hi", C.c_float * MAX_NPAR),
+                ("log_scale", C.c_uint8 * MAX_NPAR), ("periodic", C.c_uint8 * MAX_NPAR),
                 ("stokes_weight", C.c_float * 4), ("mu", C.c_void_p), ("pixel_id_base", C.c_int64)]
 
 
@@ -84,8 +85,10 @@ def _dev(t, dtype, name):
 class LineData:
     """Host-side line list. lines: list of dict(lambda0, strength, shift[], weight[], kind[])."""
 
-    def __init__(self, lines, lambda_ref, n_params=NPAR):
-        self._keep = []
+    def __init__(self, lines, lambda_ref, n_params=NPAR, nm_profile=None):
+        """n_params = 11 needs nm_profile: a contiguous CUDA f32 tensor [L] (I_fixed, reading F13)."""
+        self._keep = [nm_profile]
+        self.n_params = int(n_params)
         arr = (_MeLine * len(lines))()
         for i, l in enumerate(lines):
             sh = np.ascontiguousarray(l["shift"], dtype=np.float32)
@@ -96,7 +99,11 @@ class LineData:
                              sh.ctypes.data_as(C.POINTER(C.c_float)), we.ctypes.data_as(C.POINTER(C.c_float)),
                              ki.ctypes.data_as(C.POINTER(C.c_int8)))
         self._arr = arr
-        self.c = _MeLineData(len(lines), arr, float(lambda_ref), int(n_params), None)
+        nm_ptr = None
+        if nm_profile is not None:
+            import torch
+            nm_ptr = _dev(nm_profile, torch.float32, "nm_profile").value
+        self.c = _MeLineData(len(lines), arr, float(lambda_ref), int(n_params), nm_ptr)
 
 
 def zeeman_pattern(lower, upper):
@@ -111,7 +118,7 @@ def zeeman_pattern(lower, upper):
     return sh[:n].copy(), we[:n].copy(), ki[:n].copy()
 
 
-def line_data_from_workload(lines, triplets=True, lambda_ref=None):
+def line_data_from_workload(lines, triplets=True, lambda_ref=None, n_params=NPAR, nm_profile=None):
     """Builds a LineData from workloads.FE_* dicts: effective triplets, or the full pattern via me_zeeman_pattern."""
     from . import workloads as W
     out = []
@@ -122,7 +129,7 @@ def line_data_from_workload(lines, triplets=True, lambda_ref=None):
         else:
             sh, we, ki = zeeman_pattern(l["lower"], l["upper"])
         out.append(dict(lambda0=l["lambda0"], strength=l["strength"], shift=sh, weight=we, kind=ki))
-    return LineData(out, W.LAMBDA_REF if lambda_ref is None else lambda_ref)
+    return LineData(out, W.LAMBDA_REF if lambda_ref is None else lambda_ref, n_params, nm_profile)
 
 
 def make_ga_cfg(cfg, mu=None, pixel_id_base=0):
@@ -134,7 +141,7 @@ def make_ga_cfg(cfg, mu=None, pixel_id_base=0):
     c.p_cross, c.p_mut = cfg["p_cross"], cfg["p_mut"]
     c.mut_scale0, c.mut_scale_end = float(ms[0]), float(ms[-1])
     c.mut_scale_table = ms.ctypes.data_as(C.POINTER(C.c_float))
-    for j in range(NPAR):
+    for j in range(len(cfg["lo"])):
         c.lo[j], c.hi[j] = float(cfg["lo"][j]), float(cfg["hi"][j])
         c.log_scale[j], c.periodic[j] = int(cfg["log_scale"][j]), int(cfg["periodic"][j])
     for s in range(4):
@@ -151,9 +158,10 @@ def _grid(lam):
 
 
 def me_synth(params, lam, line_data, mu=None, out_stokes=None, obs_ref=None, w_over_sigma=None, out_chi2=None, want_stokes=True):
-    """params: CUDA f32 [P,9]. Returns (out_stokes [P,4,L] or None, out_chi2 [P] or None)."""
+    """params: CUDA f32 [P, line_data.n_params]. Returns (out_stokes [P,4,L] or None, out_chi2 [P] or None)."""
     import torch
     P = params.shape[0]
+    assert params.dim() == 2 and params.shape[1] == line_data.n_params
     lam, lam_p, L = _grid(lam)
     if out_stokes is None and want_stokes:
         out_stokes = torch.empty((P, 4, lam.size), dtype=torch.float32, device=params.device)
@@ -171,15 +179,16 @@ def me_synth(params, lam, line_data, mu=None, out_stokes=None, obs_ref=None, w_o
 
 
 def ga_invert(obs, lam, line_data, cfg, seed, mask=None, mu=None, pixel_id_base=0, out_params=None, out_chi2=None):
-    """obs: CUDA f32 [N,4,L]. Returns (out_params [N,9], out_chi2 [N])."""
+    """obs: CUDA f32 [N,4,L]. Returns (out_params [N, n_params], out_chi2 [N])."""
     import torch
     N = obs.shape[0]
     lam, lam_p, L = _grid(lam)
     assert tuple(obs.shape) == (N, 4, lam.size)
+    assert len(cfg["lo"]) == line_data.n_params
     c, keep = make_ga_cfg(cfg, mu, pixel_id_base)
     sig = np.ascontiguousarray(cfg["sigma"], dtype=np.float32)
     if out_params is None:
-        out_params = torch.empty((N, NPAR), dtype=torch.float32, device=obs.device)
+        out_params = torch.empty((N, line_data.n_params), dtype=torch.float32, device=obs.device)
     if out_chi2 is None:
         out_chi2 = torch.empty((N,), dtype=torch.float32, device=obs.device)
     _check(lib().ga_invert(_dev(obs, torch.float32, "obs"), C.c_int64(N), _dev(mask, torch.uint8, "mask"),
@@ -194,7 +203,7 @@ def ga_fitness(genes, obs, lam, line_data, cfg, mu=None):
     N, pop = genes.shape[0], genes.shape[1]
     lam, lam_p, L = _grid(lam)
     c, keep = make_ga_cfg(cfg, mu)
-    assert pop == cfg["pop"]
+    assert pop == cfg["pop"] and genes.shape[2] == line_data.n_params == len(cfg["lo"])
     sig = np.ascontiguousarray(cfg["sigma"], dtype=np.float32)
     out = torch.empty((N, pop), dtype=torch.float32, device=genes.device)
     _check(lib().ga_fitness(_dev(genes, torch.float32, "genes"), _dev(obs, torch.float32, "obs"), C.c_int64(N),
@@ -210,7 +219,7 @@ def ga_step(genes, chi2, t, cfg, seed, pixel_id_base=0):
     c, keep = make_ga_cfg(cfg, None, pixel_id_base)
     out = torch.empty_like(genes)
     _check(lib().ga_step(_dev(genes, torch.float32, "genes_in"), _dev(chi2, torch.float32, "chi2_in"), C.c_int64(N),
-                         C.c_int(t), C.byref(c), C.c_int(NPAR), C.c_uint64(seed), _dev(out, torch.float32, "genes_out"),
+                         C.c_int(t), C.byref(c), C.c_int(genes.shape[2]), C.c_uint64(seed), _dev(out, torch.float32, "genes_out"),
                          _stream()), "ga_step")
     return out
 
@@ -218,8 +227,9 @@ def ga_step(genes, chi2, t, cfg, seed, pixel_id_base=0):
 def ga_init(N, cfg, seed, pixel_id_base=0, device="cuda"):
     import torch
     c, keep = make_ga_cfg(cfg, None, pixel_id_base)
-    out = torch.empty((N, cfg["pop"], NPAR), dtype=torch.float32, device=device)
-    _check(lib().ga_init(C.c_int64(N), C.byref(c), C.c_uint64(seed), _dev(out, torch.float32, "genes_out"), _stream()), "ga_init")
+    npar = len(cfg["lo"])
+    out = torch.empty((N, cfg["pop"], npar), dtype=torch.float32, device=device)
+    _check(lib().ga_init(C.c_int64(N), C.byref(c), C.c_int(npar), C.c_uint64(seed), _dev(out, torch.float32, "genes_out"), _stream()), "ga_init")
     return out
 
 

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libme_b200.so")
-SOURCES = ["me_api.cu", "me_kernels.cu", "me_probe.cu"] + ["me_inst_%d_%s.cu" % (nl, t) for nl in (2, 1, 4) for t in ("t", "g")]
+SOURCES = ["me_api.cu", "me_kernels.cu", "me_probe.cu"] + ["me_inst_%d_%s_%d.cu" % (nl, t, m) for m in (9, 11) for nl in (2, 1, 4) for t in ("t", "g")]
 HEADERS = ["me_device.cuh", "me_inst.cuh", "me_launch.h", "faddeeva_table.h", os.path.join("..", "..", "include", "me.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xptxas=-v",
               "-Xcompiler", "-fPIC"]

@@ -24,12 +24,13 @@ int build_synth_desc(const double* lambda, int L, const me_line_data* ld, me::Sy
     if (lambda == nullptr || ld == nullptr || ld->lines == nullptr) return ME_ERR_NULL;
     if (L < 2 || L > ME_MAX_L) return ME_ERR_SHAPE;
     if (ld->n_lines < 1 || ld->n_lines > ME_MAX_LINES) return ME_ERR_SHAPE;
-    if (ld->n_params == 11) return ME_ERR_UNSUPPORTED;
-    if (ld->n_params != ME_NPAR) return ME_ERR_SHAPE;
-    if (ld->nm_profile != nullptr) return ME_ERR_UNSUPPORTED;
+    if (ld->n_params != ME_NPAR && ld->n_params != ME_MAX_NPAR) return ME_ERR_SHAPE;
+    if (ld->n_params == ME_MAX_NPAR && ld->nm_profile == nullptr) return ME_ERR_NULL;   // reading F13 needs I_fixed
+    if (ld->n_params == ME_NPAR && ld->nm_profile != nullptr) return ME_ERR_SHAPE;
     if (!(ld->lambda_ref_A > 0.0)) return ME_ERR_RANGE;
     std::memset(&d, 0, sizeof(d));
     d.L = L; d.n_lines = ld->n_lines; d.all_triplets = 1;
+    d.npar = ld->n_params; d.nm_profile = ld->nm_profile;
     int o = 0;
     for (int l = 0; l < ld->n_lines; ++l) {
         const me_line& ln = ld->lines[l];
@@ -62,8 +63,10 @@ int build_synth_desc(const double* lambda, int L, const me_line_data* ld, me::Sy
     return ME_OK;
 }
 
-int build_ga_desc(const ga_cfg* c, const float* sigma, int L, uint64_t seed, int64_t N, bool need_sigma, me::GaDesc& g) {
+int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t seed, int64_t N, bool need_sigma,
+                  me::GaDesc& g) {
     if (c == nullptr) return ME_ERR_NULL;
+    if (npar != ME_NPAR && npar != ME_MAX_NPAR) return ME_ERR_SHAPE;
     if (need_sigma && sigma == nullptr) return ME_ERR_NULL;
     if (c->pop < 2 || c->pop > ME_MAX_POP) return ME_ERR_SHAPE;
     if (c->generations < 0 || c->generations > ME_MAX_GEN) return ME_ERR_SHAPE;
@@ -76,14 +79,14 @@ int build_ga_desc(const ga_cfg* c, const float* sigma, int L, uint64_t seed, int
     g.p_cross = c->p_cross; g.p_mut = c->p_mut;
     g.key0 = (uint32_t)(seed & 0xffffffffu); g.key1 = (uint32_t)(seed >> 32);
     g.pixel_base = (uint32_t)c->pixel_id_base;
-    g.inv_nu = (float)(1.0 / (4.0 * L - ME_NPAR));
+    g.inv_nu = (float)(1.0 / (4.0 * L - npar));          // nu = 4 N_lambda - M
     for (int s = 0; s < 4; ++s) {
         double sg = need_sigma ? (double)sigma[s] : 1.0;
         if (!(sg > 0.0) || !(c->stokes_weight[s] >= 0.f)) return ME_ERR_RANGE;
         double w = (double)c->stokes_weight[s] / sg;
         g.w2[s] = (float)(w * w);
     }
-    for (int j = 0; j < ME_NPAR; ++j) {
+    for (int j = 0; j < npar; ++j) {
         if (!(c->lo[j] <= c->hi[j])) return ME_ERR_RANGE;
         g.lo[j] = c->lo[j];
         g.span[j] = (float)((double)c->hi[j] - (double)c->lo[j]);
@@ -109,7 +112,7 @@ int build_ga_desc(const ga_cfg* c, const float* sigma, int L, uint64_t seed, int
 
 extern "C" {
 
-int me_version(void) { return 100; }
+int me_version(void) { return 110; }
 
 const char* me_last_cuda_error(void) { return g_cuda_err.c_str(); }
 
@@ -142,7 +145,7 @@ int me_synth(const float* params, int64_t P, const float* mu, const double* lamb
             if (!(w_over_sigma[s] >= 0.f)) return ME_ERR_RANGE;
             w2[s] = w_over_sigma[s] * w_over_sigma[s];
         }
-    cudaError_t e = me::launch_synth(sd, params, mu, P, out_stokes, obs_ref, w2, (float)(1.0 / (4.0 * L - ME_NPAR)),
+    cudaError_t e = me::launch_synth(sd, params, mu, P, out_stokes, obs_ref, w2, (float)(1.0 / (4.0 * L - sd.npar)),
                                      out_chi2, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
@@ -153,7 +156,7 @@ int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sig
     me::SynthDesc sd; me::GaDesc gd;
     int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
     if (rc != ME_OK) return rc;
-    rc = build_ga_desc(cfg, sigma, L, seed, N, true, gd);
+    rc = build_ga_desc(cfg, sd.npar, sigma, L, seed, N, true, gd);
     if (rc != ME_OK) return rc;
     if (N == 0) return ME_OK;
     if (obs == nullptr || out_params == nullptr || out_chi2 == nullptr) return ME_ERR_NULL;
@@ -166,7 +169,7 @@ int ga_fitness(const float* genes, const float* obs, int64_t N, const float* sig
     me::SynthDesc sd; me::GaDesc gd;
     int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
     if (rc != ME_OK) return rc;
-    rc = build_ga_desc(cfg, sigma, L, 0, N, true, gd);
+    rc = build_ga_desc(cfg, sd.npar, sigma, L, 0, N, true, gd);
     if (rc != ME_OK) return rc;
     if (N == 0) return ME_OK;
     if (genes == nullptr || obs == nullptr || chi2_out == nullptr) return ME_ERR_NULL;
@@ -176,25 +179,23 @@ int ga_fitness(const float* genes, const float* obs, int64_t N, const float* sig
 
 int ga_step(const float* genes_in, const float* chi2_in, int64_t N, int generation, const ga_cfg* cfg, int n_params,
             uint64_t seed, float* genes_out, void* stream) {
-    if (n_params == 11) return ME_ERR_UNSUPPORTED;
-    if (n_params != ME_NPAR) return ME_ERR_SHAPE;
     me::GaDesc gd;
-    int rc = build_ga_desc(cfg, nullptr, 4, seed, N, false, gd);
+    int rc = build_ga_desc(cfg, n_params, nullptr, 4, seed, N, false, gd);
     if (rc != ME_OK) return rc;
     if (generation < 1 || generation > cfg->generations) return ME_ERR_RANGE;
     if (N == 0) return ME_OK;
     if (genes_in == nullptr || chi2_in == nullptr || genes_out == nullptr) return ME_ERR_NULL;
-    cudaError_t e = me::launch_ga_step(gd, genes_in, chi2_in, N, generation, genes_out, (cudaStream_t)stream);
+    cudaError_t e = me::launch_ga_step(gd, n_params, genes_in, chi2_in, N, generation, genes_out, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 
-int ga_init(int64_t N, const ga_cfg* cfg, uint64_t seed, float* genes_out, void* stream) {
+int ga_init(int64_t N, const ga_cfg* cfg, int n_params, uint64_t seed, float* genes_out, void* stream) {
     me::GaDesc gd;
-    int rc = build_ga_desc(cfg, nullptr, 4, seed, N, false, gd);
+    int rc = build_ga_desc(cfg, n_params, nullptr, 4, seed, N, false, gd);
     if (rc != ME_OK) return rc;
     if (N == 0) return ME_OK;
     if (genes_out == nullptr) return ME_ERR_NULL;
-    cudaError_t e = me::launch_ga_init(gd, N, genes_out, (cudaStream_t)stream);
+    cudaError_t e = me::launch_ga_init(gd, n_params, N, genes_out, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 

@@ -33,6 +33,8 @@ struct LineDesc {
 
 struct alignas(16) SynthDesc {
     int L, n_lines, n_comp, all_triplets;
+    int npar, pad0;                       // 9, or 11 (fill fraction + stray light, reading F13)
+    const float* nm_profile;              // device [L]: I_fixed of the 11-parameter model, else nullptr
     LineDesc line[ME_MAX_LINES];
     float shift[ME_MAX_COMP];
     float weight[ME_MAX_COMP];
@@ -46,8 +48,8 @@ struct GaDesc {
     uint32_t pixel_base;
     float inv_nu;                       // 1 / (4L - M)
     float w2[4];                        // (w_s / sigma_s)^2
-    float lo[ME_NPAR], span[ME_NPAR], log2ratio[ME_NPAR];
-    int log_scale[ME_NPAR], periodic[ME_NPAR];
+    float lo[ME_MAX_NPAR], span[ME_MAX_NPAR], log2ratio[ME_MAX_NPAR];
+    int log_scale[ME_MAX_NPAR], periodic[ME_MAX_NPAR];
     float mut_scale[ME_MAX_GEN + 1];    // s_t, t = 0..generations
 };
 
@@ -193,10 +195,15 @@ struct Individual {
     float invD[NL], v0[NL], vB[NL];   // 1/dlambdaD_l, -doppler_l/dlambdaD_l, Zeeman splitting in Doppler units
     float kA, kB, kC;                 // h sin^2(gamma), h (1 + cos^2 gamma)/2, h cos(gamma);  h = eta0 / (2 sqrt(pi))
     float c2x, s2x;                   // cos 2chi, sin 2chi
-    float S0, muS1;
+    float S0, muS1;                   // 11-parameter model: (1-s) S0 and (1-s) alpha mu S1
+    float k0, nmS1, stray;            // 11-parameter model only: eta0/sqrt(pi), (1-s)(1-alpha) mu S1, s
 };
 
-template <int NL>
+// p: decoded parameter vector, M = 9 or 11 entries.  For M = 11 (reading F13)
+//   I = (1-s)[alpha I^M + (1-alpha) I(B=0)] + s I_fixed
+//     = (1-s) S0 + [(1-s) alpha mu S1] (K^-1 e)_I + [(1-s)(1-alpha) mu S1] / (1 + eta0 phi_nm) + s I_fixed,
+// and Q, U, V carry the factor (1-s) alpha: both are obtained by rescaling S0 and mu S1 here.
+template <int NL, int M>
 MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const SynthDesc& d) {
     const float B = p[0], eta0 = p[3], dld = p[4], a = p[5], vlos = p[6];
     float sg, cg;
@@ -210,6 +217,15 @@ MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const
     ind.far2 = a <= FAD_FAR_AMAX ? FAD_FAR2 : __int_as_float(0x7f800000);
     ind.S0 = p[7];
     ind.muS1 = mu * p[8];
+    ind.k0 = ind.nmS1 = ind.stray = 0.f;
+    if (M == ME_MAX_NPAR) {
+        const float alpha = p[9], s = p[10], oms = 1.0f - s;
+        ind.k0 = 2.0f * h;
+        ind.nmS1 = oms * (1.0f - alpha) * ind.muS1;
+        ind.muS1 = oms * alpha * ind.muS1;
+        ind.S0 = oms * ind.S0;
+        ind.stray = s;
+    }
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
         if (NL == ME_MAX_LINES && l >= d.n_lines) { ind.invD[l] = ind.v0[l] = ind.vB[l] = 0.f; ind.far[l] = far_coef(a, 0.f); continue; }
@@ -281,16 +297,24 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
 // Stokes vectors at the wavelength pair (j0, j1) (eq. 8 + eq. 12-13 times I_c of eq. 15).  j1 = j0 + 1 with j0 even
 // in the main loop (one 8-byte constant-bank load per line); j1 = j0 for the odd tail.
 // The Unno-Rachkovsky solution is evaluated in the frame chi = 0 (eta_U = rho_U = 0) and Q,U are rotated by 2 chi.
-template <int NL, bool TRIPLET>
-MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2& I, f2& Q, f2& U, f2& V) {
-    f2 br = bc(0.f), bi = bc(0.f), pr = bc(0.f), pi = bc(0.f), rr = bc(0.f), ri = bc(0.f);
+// M = 11: nmF = I_fixed at the two wavelengths; the field-free profile sum phi_nm = sum_l r_l H(a, v_l) is the pi sum of
+// effective triplets (their pi component is unshifted with weight 1), else one extra Voigt per line.
+template <int NL, bool TRIPLET, int M>
+MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2 nmF, f2& I, f2& Q, f2& U, f2& V) {
+    f2 br = bc(0.f), bi = bc(0.f), pr = bc(0.f), pi = bc(0.f), rr = bc(0.f), ri = bc(0.f), nr = bc(0.f);
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
         if (NL == ME_MAX_LINES && l >= d.n_lines) break;      // NL == ME_MAX_LINES is the run-time-sized fallback
         const f2 off = tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]);
         const f2 v = fma2(ind.invD[l], off, ind.v0[l]);
         line_profiles<TRIPLET>(v, ind.vB[l], ind.fad, ind.far[l], ind.far2, d, l, br, bi, pr, pi, rr, ri);
+        if (M == ME_MAX_NPAR && !TRIPLET) {
+            f2 wr, wi;
+            faddeeva_pair(v, ind.fad, wr, wi);
+            nr = fma2(d.line[l].strength, wr, nr);
+        }
     }
+    if (M == ME_MAX_NPAR && TRIPLET) nr = pr;
     const f2 sr = add2(br, rr), si = add2(bi, ri);                // sigma sums
     const f2 eI = fma2(ind.kA, pr, fma2(ind.kB, sr, 1.0f));
     const f2 eL = mul2(ind.kA, fma2(-0.5f, sr, pr));              // eta_Q in the chi = 0 frame
@@ -309,6 +333,10 @@ MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bo
     V = mul2(nt, fma2(eI2, eV, mul2(rV, Pi)));
     Q = fma2(ind.c2x, Qp, mul2(-ind.s2x, Up));
     U = fma2(ind.s2x, Qp, mul2(ind.c2x, Up));
+    if (M == ME_MAX_NPAR) {
+        const f2 rn = rcp2(fma2(ind.k0, nr, 1.0f));               // 1 / (1 + eta0 phi_nm): pin P1
+        I = fma2(ind.nmS1, rn, fma2(ind.stray, nmF, I));
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -345,13 +373,14 @@ __device__ __forceinline__ float decode_gene(float g, const GaDesc& c, int j) {
 }
 
 // generation 0, gene j: lane (j mod 4) of block floor(j / 4)
+template <int M>
 __device__ __forceinline__ void init_genes(float* g, uint32_t pixel, uint32_t i, const GaDesc& c) {
 #pragma unroll
-    for (int k = 0; k < (ME_NPAR + 3) / 4; ++k) {
+    for (int k = 0; k < (M + 3) / 4; ++k) {
         const uint4 r = philox4x32_10(pixel, 0u, i, (uint32_t)k, c.key0, c.key1);
 #pragma unroll
         for (int q = 0; q < 4; ++q)
-            if (4 * k + q < ME_NPAR) g[4 * k + q] = u01(lane_of(r, q));
+            if (4 * k + q < M) g[4 * k + q] = u01(lane_of(r, q));
     }
 }
 
@@ -367,7 +396,8 @@ __device__ __forceinline__ int tournament(const uint4& r, const float* chi2, con
     return best;
 }
 
-// Child i >= 1 of generation t from the previous population `genes` [pop][ME_NPAR] and its fitness `chi2` [pop].
+// Child i >= 1 of generation t from the previous population `genes` [pop][M] and its fitness `chi2` [pop].
+template <int M>
 __device__ __forceinline__ void make_child(float* child, const float* genes, const float* chi2, uint32_t pixel,
                                            uint32_t t, uint32_t i, float s_t, const GaDesc& c) {
     const int A = tournament(philox4x32_10(pixel, t, i, 0u, c.key0, c.key1), chi2, c);
@@ -377,8 +407,8 @@ __device__ __forceinline__ void make_child(float* child, const float* genes, con
     const float alpha = u01(rc.y);
     uint4 rm = make_uint4(0, 0, 0, 0);
 #pragma unroll
-    for (int j = 0; j < ME_NPAR; ++j) {
-        const float gA = genes[A * ME_NPAR + j], gB = genes[B * ME_NPAR + j];
+    for (int j = 0; j < M; ++j) {
+        const float gA = genes[A * M + j], gB = genes[B * M + j];
         float g = gA;
         if (cross) g = __fmaf_rn(alpha, __fsub_rn(gA, gB), gB);
         if ((j & 1) == 0) rm = philox4x32_10(pixel, t, i, (uint32_t)(3 + j / 2), c.key0, c.key1);

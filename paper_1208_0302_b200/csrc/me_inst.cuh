@@ -10,20 +10,21 @@ namespace me {
 // ------------------------------------------------------------------------------------------------------------
 // Fitness of one individual held in registers: decode -> per-individual constants -> wavelength loop.
 // obs_s: shared memory, per wavelength pair two float4 = (I0,I1,Q0,Q1), (U0,U1,V0,V1) (broadcast reads, conflict-free).
+// nm_s:  shared memory, per wavelength pair one float2 of I_fixed (M = 11 only).
 // ------------------------------------------------------------------------------------------------------------
-template <int NL, bool TRIPLET>
+template <int NL, bool TRIPLET, int M>
 __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
-                                         const float4* obs_s) {
-    float p[ME_NPAR];
+                                         const float4* obs_s, const float2* nm_s) {
+    float p[M];
 #pragma unroll
-    for (int j = 0; j < ME_NPAR; ++j) p[j] = decode_gene(g[j], gd, j);
+    for (int j = 0; j < M; ++j) p[j] = decode_gene(g[j], gd, j);
     Individual<NL> ind;
-    setup_individual<NL>(ind, p, mu, sd);
+    setup_individual<NL, M>(ind, p, mu, sd);
     f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
     const int L = sd.L, npair = L >> 1;
     for (int jp = 0; jp < npair; ++jp) {
         f2 I, Q, U, V;
-        stokes_pair<NL, TRIPLET>(ind, sd, 2 * jp, false, I, Q, U, V);
+        stokes_pair<NL, TRIPLET, M>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V);
         const float4 o0 = obs_s[2 * jp], o1 = obs_s[2 * jp + 1];           // (I0,I1,Q0,Q1), (U0,U1,V0,V1)
         const f2 dI = sub2(make_float2(o0.x, o0.y), I), dQ = sub2(make_float2(o0.z, o0.w), Q);
         const f2 dU = sub2(make_float2(o1.x, o1.y), U), dV = sub2(make_float2(o1.z, o1.w), V);
@@ -31,7 +32,7 @@ __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDe
     }
     if (L & 1) {                                                            // odd tail: second half is a duplicate, dropped
         f2 I, Q, U, V;
-        stokes_pair<NL, TRIPLET>(ind, sd, L - 1, true, I, Q, U, V);
+        stokes_pair<NL, TRIPLET, M>(ind, sd, L - 1, true, M == ME_MAX_NPAR ? nm_s[npair] : bc(0.f), I, Q, U, V);
         const float4 o0 = obs_s[2 * npair], o1 = obs_s[2 * npair + 1];
         const float dI = o0.x - I.x, dQ = o0.z - Q.x, dU = o1.x - U.x, dV = o1.z - V.x;
         aI.x = fmaf(dI, dI, aI.x); aQ.x = fmaf(dQ, dQ, aQ.x); aU.x = fmaf(dU, dU, aU.x); aV.x = fmaf(dV, dV, aV.x);
@@ -51,11 +52,19 @@ __device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int 
     }
 }
 
+// Stage I_fixed[L] pair-wise: nm_s[jp] = (F[2jp], F[2jp+1]); the odd tail duplicates its single value.
+__device__ __forceinline__ void stage_nm(float2* nm_s, const float* nm, int L, int tid, int nthreads) {
+    for (int jp = tid; jp < (L + 1) / 2; jp += nthreads) {
+        const float a = __ldg(nm + 2 * jp), b = 2 * jp + 1 < L ? __ldg(nm + 2 * jp + 1) : a;
+        nm_s[jp] = make_float2(a, b);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // The fused GA inversion kernel.
-// Dynamic shared memory: obs_s [ceil(L/2)] 2 x float4 | genes [2][pop][9] | chi2 [2][pop] | scratch [64]
+// Dynamic shared memory: obs_s [ceil(L/2)] 2 x float4 | nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] | scratch [64]
 // ------------------------------------------------------------------------------------------------------------
-template <int NL, bool TRIPLET, int THREADS, int MINB>
+template <int NL, bool TRIPLET, int M, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
 ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
                  const float* __restrict__ obs, const uint8_t* __restrict__ mask, const float* __restrict__ mu_arr,
@@ -63,8 +72,10 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
     extern __shared__ float4 smem4[];
     const int L = sd.L, pop = gd.pop;
     float* obs_s = reinterpret_cast<float*>(smem4);
-    float* genes_s = obs_s + 8 * ((L + 1) >> 1);
-    float* chi2_s = genes_s + 2 * pop * ME_NPAR;
+    float2* nm_s = reinterpret_cast<float2*>(obs_s + 8 * ((L + 1) >> 1));
+    float* genes_s = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));
+    float* chi2_s = genes_s + 2 * pop * M;
+    if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, threadIdx.x, THREADS);     // once per CTA; synced below
     uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + 2 * pop);
     const int tid = threadIdx.x;
     const float INF = __int_as_float(0x7f800000);
@@ -72,7 +83,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
     for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
         if (mask != nullptr && mask[n] == 0) {
             const float qnan = __int_as_float(0x7fc00000);
-            if (tid < ME_NPAR) out_params[n * ME_NPAR + tid] = qnan;
+            if (tid < M) out_params[n * M + tid] = qnan;
             if (tid == 0) out_chi2[n] = qnan;
             continue;
         }
@@ -82,7 +93,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
 
         // generations 0..G with ONE fitness call site (keeps the loop body inside the instruction cache)
-        float g[ME_NPAR];
+        float g[M];
         float f = INF;
         int cur = 1;                                       // generation t reads buffer cur, writes cur ^ 1
         const bool alive = tid < pop;
@@ -90,24 +101,24 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
             float fe = INF; int ie = 0;
             if (t > 0) block_argmin(f, tid, scratch, fe, ie);   // elite of generation t-1
             else __syncthreads();                          // obs staged
-            const float* gprev = genes_s + cur * pop * ME_NPAR;
+            const float* gprev = genes_s + cur * pop * M;
             const float* fprev = chi2_s + cur * pop;
-            float* gnext = genes_s + (cur ^ 1) * pop * ME_NPAR;
+            float* gnext = genes_s + (cur ^ 1) * pop * M;
             if (alive) {
                 bool evaluate = true;
                 if (t == 0) {
-                    init_genes(g, pixel, (uint32_t)tid, gd);                       // reading G2
+                    init_genes<M>(g, pixel, (uint32_t)tid, gd);                       // reading G2
                 } else if (tid == 0) {
 #pragma unroll
-                    for (int j = 0; j < ME_NPAR; ++j) g[j] = gprev[ie * ME_NPAR + j];
+                    for (int j = 0; j < M; ++j) g[j] = gprev[ie * M + j];
                     f = fe;                                // carried, not re-evaluated (reading G3)
                     evaluate = false;
                 } else {
-                    make_child(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
+                    make_child<M>(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
                 }
-                if (evaluate) f = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
+                if (evaluate) f = fitness<NL, TRIPLET, M>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s);
 #pragma unroll
-                for (int j = 0; j < ME_NPAR; ++j) gnext[tid * ME_NPAR + j] = g[j];
+                for (int j = 0; j < M; ++j) gnext[tid * M + j] = g[j];
                 chi2_s[(cur ^ 1) * pop + tid] = f;
             }
             cur ^= 1;
@@ -118,7 +129,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         block_argmin(f, tid, scratch, fe, ie);             // reading G5
         if (tid == ie) {
 #pragma unroll
-            for (int j = 0; j < ME_NPAR; ++j) out_params[n * ME_NPAR + j] = decode_gene(g[j], gd, j);
+            for (int j = 0; j < M; ++j) out_params[n * M + j] = decode_gene(g[j], gd, j);
             out_chi2[n] = f;
         }
     }
@@ -137,7 +148,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 #define SYNTH_VS (4 * SYNTH_CW + 4)      /* row stride: 16-byte aligned rows for LDS.128 / STG.128 */
 #define SYNTH_THREADS 128
 
-template <int NL, bool TRIPLET>
+template <int NL, bool TRIPLET, int M>
 __global__ void __launch_bounds__(SYNTH_THREADS, 4)
 me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
                 int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
@@ -151,19 +162,21 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
         const int64_t wbase = base + warp * 32;                 // first vector of this warp
         if (wbase >= P) continue;
         const int64_t v = wbase + lane < P ? wbase + lane : P - 1;   // idle lanes recompute the last vector, never store
-        float p[ME_NPAR];
+        float p[M];
 #pragma unroll
-        for (int j = 0; j < ME_NPAR; ++j) p[j] = __ldg(params + v * ME_NPAR + j);
+        for (int j = 0; j < M; ++j) p[j] = __ldg(params + v * M + j);
         const float mu = mu_arr != nullptr ? __ldg(mu_arr + v) : 1.0f;
         Individual<NL> ind;
-        setup_individual<NL>(ind, p, mu, sd);
+        setup_individual<NL, M>(ind, p, mu, sd);
+        const float* nm = sd.nm_profile;
         f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
         for (int jp0 = 0; jp0 < npair; jp0 += SYNTH_CW / 2) {
             const int nloc = min(SYNTH_CW / 2, npair - jp0);
             for (int i = 0; i < nloc; ++i) {
                 const int j = 2 * (jp0 + i);
                 f2 I, Q, U, V;
-                stokes_pair<NL, TRIPLET>(ind, sd, j, false, I, Q, U, V);
+                const f2 nmF = M == ME_MAX_NPAR ? make_float2(__ldg(nm + j), __ldg(nm + j + 1)) : bc(0.f);
+                stokes_pair<NL, TRIPLET, M>(ind, sd, j, false, nmF, I, Q, U, V);
                 if (want_out) {
                     float2* t = reinterpret_cast<float2*>(tile + lane * SYNTH_VS + 2 * i);
                     t[0] = I; t[SYNTH_CW / 2] = Q; t[SYNTH_CW] = U; t[3 * SYNTH_CW / 2] = V;
@@ -203,7 +216,7 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
         }
         if (L & 1) {                                             // odd tail: one wavelength, written directly
             f2 I, Q, U, V;
-            stokes_pair<NL, TRIPLET>(ind, sd, L - 1, true, I, Q, U, V);
+            stokes_pair<NL, TRIPLET, M>(ind, sd, L - 1, true, M == ME_MAX_NPAR ? bc(__ldg(nm + L - 1)) : bc(0.f), I, Q, U, V);
             if (want_out && wbase + lane < P) {
                 float* o = out_stokes + v * 4 * (int64_t)L + (L - 1);
                 __stcs(o, I.x); __stcs(o + L, Q.x); __stcs(o + 2 * L, U.x); __stcs(o + 3 * L, V.x);
@@ -222,7 +235,7 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
 }
 
 // Test hook: the fused fitness alone (128 threads per pixel, individuals strided over the block).
-template <int NL, bool TRIPLET>
+template <int NL, bool TRIPLET, int M>
 __global__ void __launch_bounds__(128, 4)
 ga_fitness_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
                   const float* __restrict__ genes, const float* __restrict__ obs, const float* __restrict__ mu_arr,
@@ -230,16 +243,18 @@ ga_fitness_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ 
     extern __shared__ float4 smem4[];
     float* obs_s = reinterpret_cast<float*>(smem4);
     const int L = sd.L, pop = gd.pop, tid = threadIdx.x;
+    float2* nm_s = reinterpret_cast<float2*>(obs_s + 8 * ((L + 1) >> 1));
+    if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, tid, 128);
     for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
         __syncthreads();
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, 128);
         __syncthreads();
         const float mu = mu_arr != nullptr ? __ldg(mu_arr + n) : 1.0f;
         for (int i = tid; i < pop; i += 128) {
-            float g[ME_NPAR];
+            float g[M];
 #pragma unroll
-            for (int j = 0; j < ME_NPAR; ++j) g[j] = genes[(n * pop + i) * ME_NPAR + j];
-            chi2_out[n * pop + i] = fitness<NL, TRIPLET>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s));
+            for (int j = 0; j < M; ++j) g[j] = genes[(n * pop + i) * M + j];
+            chi2_out[n * pop + i] = fitness<NL, TRIPLET, M>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s);
         }
     }
 }
@@ -249,11 +264,11 @@ ga_fitness_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ 
 // ------------------------------------------------------------------------------------------------------------
 static inline unsigned grid_for_(int64_t n) { return (unsigned)(n < 0x7fffffffLL ? n : 0x7fffffffLL); }
 
-template <int NL, bool TRIPLET, int THREADS, int MINB>
+template <int NL, bool TRIPLET, int M, int THREADS, int MINB>
 static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask,
                                       const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
-    auto k = ga_invert_kernel<NL, TRIPLET, THREADS, MINB>;
-    const size_t smem = (size_t)32 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * ME_NPAR * 4 + (size_t)2 * gd.pop * 4 + 64 * 4;
+    auto k = ga_invert_kernel<NL, TRIPLET, M, THREADS, MINB>;
+    const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * M * 4 + (size_t)2 * gd.pop * 4 + 64 * 4;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid_for_(N), THREADS, smem, st>>>(sd, gd, obs, mask, mu, N, out_params, out_chi2);
@@ -264,16 +279,16 @@ static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, con
 #define ME_DISPATCH_THREADS(FN, ...)                                                                          \
     do {                                                                                                        \
         const int pop_ = gd.pop;                                                                                \
-        if (pop_ <= 64) return FN<ME_INST_NL, ME_INST_TRIPLET, 64, 8>(__VA_ARGS__);                             \
-        if (pop_ <= 128) return FN<ME_INST_NL, ME_INST_TRIPLET, 128, 4>(__VA_ARGS__);                           \
-        if (pop_ <= 256) return FN<ME_INST_NL, ME_INST_TRIPLET, 256, 2>(__VA_ARGS__);                           \
-        if (pop_ <= 512) return FN<ME_INST_NL, ME_INST_TRIPLET, 512, 1>(__VA_ARGS__);                           \
-        return FN<ME_INST_NL, ME_INST_TRIPLET, 1024, 1>(__VA_ARGS__);                                           \
+        if (pop_ <= 64) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 64, 8>(__VA_ARGS__);                  \
+        if (pop_ <= 128) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 128, 4>(__VA_ARGS__);                \
+        if (pop_ <= 256) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 256, 2>(__VA_ARGS__);                \
+        if (pop_ <= 512) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 512, 1>(__VA_ARGS__);                \
+        return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 1024, 1>(__VA_ARGS__);                                \
     } while (0)
 
-#define ME_CAT3_(a, b, c) a##_##b##_##c
-#define ME_CAT3(a, b, c) ME_CAT3_(a, b, c)
-#define ME_INST_NAME(base) ME_CAT3(base, ME_INST_NL, ME_INST_TAG)
+#define ME_CAT4_(a, b, c, d) a##_##b##_##c##_##d
+#define ME_CAT4(a, b, c, d) ME_CAT4_(a, b, c, d)
+#define ME_INST_NAME(base) ME_CAT4(base, ME_INST_NL, ME_INST_TAG, ME_INST_M)
 
 cudaError_t ME_INST_NAME(launch_ga_invert)(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask,
                                            const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
@@ -282,8 +297,8 @@ cudaError_t ME_INST_NAME(launch_ga_invert)(const SynthDesc& sd, const GaDesc& gd
 
 cudaError_t ME_INST_NAME(launch_ga_fitness)(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs,
                                             const float* mu, int64_t N, float* chi2_out, cudaStream_t st) {
-    const size_t smem = (size_t)32 * ((sd.L + 1) / 2);
-    ga_fitness_kernel<ME_INST_NL, ME_INST_TRIPLET><<<grid_for_(N), 128, smem, st>>>(sd, gd, genes, obs, mu, N, chi2_out);
+    const size_t smem = (size_t)40 * ((sd.L + 1) / 2);
+    ga_fitness_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid_for_(N), 128, smem, st>>>(sd, gd, genes, obs, mu, N, chi2_out);
     return cudaGetLastError();
 }
 
@@ -297,7 +312,7 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
     const int64_t cap = (int64_t)sms * 4;                            // persistent grid: 4 resident blocks per SM
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
     const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float);
-    me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET><<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, P, out_stokes, obs_ref, w2[0],
+    me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, P, out_stokes, obs_ref, w2[0],
                                                                                    w2[1], w2[2], w2[3], inv_nu, out_chi2);
     return cudaGetLastError();
 }

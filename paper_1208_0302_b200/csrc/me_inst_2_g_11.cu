@@ -1,0 +1,6 @@
+// Specialisation: 2 line(s), general component lists, 11 parameters.
+#define ME_INST_NL 2
+#define ME_INST_TRIPLET false
+#define ME_INST_TAG g
+#define ME_INST_M 11
+#include "me_inst.cuh"

@@ -1,0 +1,6 @@
+// Specialisation: up to 4 (run-time) line(s), effective triplets, 9 parameters.
+#define ME_INST_NL 4
+#define ME_INST_TRIPLET true
+#define ME_INST_TAG t
+#define ME_INST_M 9
+#include "me_inst.cuh"

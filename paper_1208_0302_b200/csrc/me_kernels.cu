@@ -18,18 +18,19 @@ namespace me {
 // ------------------------------------------------------------------------------------------------------------
 // Test hooks
 // ------------------------------------------------------------------------------------------------------------
-// One generation from given genes and given fitness (shared: genes [pop][9] | chi2 [pop] | scratch [64]).
+// One generation from given genes and given fitness (shared: genes [pop][M] | chi2 [pop] | scratch [64]).
+template <int M>
 __global__ void ga_step_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ genes_in,
                                const float* __restrict__ chi2_in, int64_t N, int t, float* __restrict__ genes_out) {
     extern __shared__ float4 smem4[];
     const int pop = gd.pop, tid = threadIdx.x;
     float* genes_s = reinterpret_cast<float*>(smem4);
-    float* chi2_s = genes_s + pop * ME_NPAR;
+    float* chi2_s = genes_s + pop * M;
     uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + pop);
     const float INF = __int_as_float(0x7f800000);
     for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
         __syncthreads();
-        for (int k = tid; k < pop * ME_NPAR; k += blockDim.x) genes_s[k] = genes_in[n * pop * ME_NPAR + k];
+        for (int k = tid; k < pop * M; k += blockDim.x) genes_s[k] = genes_in[n * pop * M + k];
         float f = INF;
         if (tid < pop) {
             f = chi2_in[n * pop + tid];
@@ -40,28 +41,29 @@ __global__ void ga_step_kernel(const __grid_constant__ GaDesc gd, const float* _
         float fe; int ie;
         block_argmin(f, tid, scratch, fe, ie);
         if (tid < pop) {
-            float g[ME_NPAR];
+            float g[M];
             if (tid == 0) {
 #pragma unroll
-                for (int j = 0; j < ME_NPAR; ++j) g[j] = genes_s[ie * ME_NPAR + j];
+                for (int j = 0; j < M; ++j) g[j] = genes_s[ie * M + j];
             } else {
-                make_child(g, genes_s, chi2_s, gd.pixel_base + (uint32_t)n, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
+                make_child<M>(g, genes_s, chi2_s, gd.pixel_base + (uint32_t)n, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
             }
 #pragma unroll
-            for (int j = 0; j < ME_NPAR; ++j) genes_out[(n * pop + tid) * ME_NPAR + j] = g[j];
+            for (int j = 0; j < M; ++j) genes_out[(n * pop + tid) * M + j] = g[j];
         }
     }
 }
 
+template <int M>
 __global__ void ga_init_kernel(const __grid_constant__ GaDesc gd, int64_t N, float* __restrict__ genes_out) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N * gd.pop) return;
     const int64_t n = k / gd.pop;
     const int i = (int)(k - n * gd.pop);
-    float g[ME_NPAR];
-    init_genes(g, gd.pixel_base + (uint32_t)n, (uint32_t)i, gd);
+    float g[M];
+    init_genes<M>(g, gd.pixel_base + (uint32_t)n, (uint32_t)i, gd);
 #pragma unroll
-    for (int j = 0; j < ME_NPAR; ++j) genes_out[k * ME_NPAR + j] = g[j];
+    for (int j = 0; j < M; ++j) genes_out[k * M + j] = g[j];
 }
 
 __global__ void philox_kernel(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -85,25 +87,31 @@ __global__ void faddeeva_kernel(const float* __restrict__ v, const float* __rest
 static inline unsigned grid_for(int64_t n) { return (unsigned)(n < 0x7fffffffLL ? n : 0x7fffffffLL); }
 
 // The heavy kernels live in me_inst_<nl>_<t|g>.cu (one translation unit per specialisation).
-#define ME_DECL_INST(NL, TAG)                                                                                            \
-    cudaError_t launch_ga_invert_##NL##_##TAG(const SynthDesc&, const GaDesc&, const float*, const uint8_t*, const float*, \
-                                              int64_t, float*, float*, cudaStream_t);                                     \
-    cudaError_t launch_ga_fitness_##NL##_##TAG(const SynthDesc&, const GaDesc&, const float*, const float*, const float*,  \
-                                               int64_t, float*, cudaStream_t);                                            \
-    cudaError_t launch_synth_##NL##_##TAG(const SynthDesc&, const float*, const float*, int64_t, float*, const float*,    \
-                                          const float*, float, float*, cudaStream_t);
-ME_DECL_INST(1, t) ME_DECL_INST(2, t) ME_DECL_INST(4, t) ME_DECL_INST(1, g) ME_DECL_INST(2, g) ME_DECL_INST(4, g)
+#define ME_DECL_INST(NL, TAG, M)                                                                                                \
+    cudaError_t launch_ga_invert_##NL##_##TAG##_##M(const SynthDesc&, const GaDesc&, const float*, const uint8_t*, const float*, \
+                                                    int64_t, float*, float*, cudaStream_t);                                     \
+    cudaError_t launch_ga_fitness_##NL##_##TAG##_##M(const SynthDesc&, const GaDesc&, const float*, const float*, const float*,  \
+                                                     int64_t, float*, cudaStream_t);                                            \
+    cudaError_t launch_synth_##NL##_##TAG##_##M(const SynthDesc&, const float*, const float*, int64_t, float*, const float*,    \
+                                                const float*, float, float*, cudaStream_t);
+ME_DECL_INST(1, t, 9) ME_DECL_INST(2, t, 9) ME_DECL_INST(4, t, 9) ME_DECL_INST(1, g, 9) ME_DECL_INST(2, g, 9) ME_DECL_INST(4, g, 9)
+ME_DECL_INST(1, t, 11) ME_DECL_INST(2, t, 11) ME_DECL_INST(4, t, 11) ME_DECL_INST(1, g, 11) ME_DECL_INST(2, g, 11) ME_DECL_INST(4, g, 11)
 
-#define ME_DISPATCH(BASE, ...)                                                       \
+#define ME_DISPATCH_M(BASE, M, ...)                                                  \
     do {                                                                             \
         if (sd.all_triplets) {                                                       \
-            if (sd.n_lines == 1) return BASE##_1_t(__VA_ARGS__);                     \
-            if (sd.n_lines == 2) return BASE##_2_t(__VA_ARGS__);                     \
-            return BASE##_4_t(__VA_ARGS__);                                          \
+            if (sd.n_lines == 1) return BASE##_1_t_##M(__VA_ARGS__);                 \
+            if (sd.n_lines == 2) return BASE##_2_t_##M(__VA_ARGS__);                 \
+            return BASE##_4_t_##M(__VA_ARGS__);                                      \
         }                                                                            \
-        if (sd.n_lines == 1) return BASE##_1_g(__VA_ARGS__);                         \
-        if (sd.n_lines == 2) return BASE##_2_g(__VA_ARGS__);                         \
-        return BASE##_4_g(__VA_ARGS__);                                              \
+        if (sd.n_lines == 1) return BASE##_1_g_##M(__VA_ARGS__);                     \
+        if (sd.n_lines == 2) return BASE##_2_g_##M(__VA_ARGS__);                     \
+        return BASE##_4_g_##M(__VA_ARGS__);                                          \
+    } while (0)
+#define ME_DISPATCH(BASE, ...)                                                       \
+    do {                                                                             \
+        if (sd.npar == ME_MAX_NPAR) ME_DISPATCH_M(BASE, 11, __VA_ARGS__);            \
+        ME_DISPATCH_M(BASE, 9, __VA_ARGS__);                                         \
     } while (0)
 
 cudaError_t launch_ga_invert(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask, const float* mu,
@@ -121,17 +129,19 @@ cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* 
     ME_DISPATCH(launch_synth, sd, params, mu, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
 }
 
-cudaError_t launch_ga_step(const GaDesc& gd, const float* genes_in, const float* chi2_in, int64_t N, int t,
+cudaError_t launch_ga_step(const GaDesc& gd, int npar, const float* genes_in, const float* chi2_in, int64_t N, int t,
                            float* genes_out, cudaStream_t st) {
     const int threads = ((gd.pop + 31) / 32) * 32;
-    const size_t smem = (size_t)gd.pop * ME_NPAR * 4 + (size_t)gd.pop * 4 + 64 * 4;
-    ga_step_kernel<<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
+    const size_t smem = (size_t)gd.pop * npar * 4 + (size_t)gd.pop * 4 + 64 * 4;
+    if (npar == ME_MAX_NPAR) ga_step_kernel<ME_MAX_NPAR><<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
+    else ga_step_kernel<ME_NPAR><<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
     return cudaGetLastError();
 }
 
-cudaError_t launch_ga_init(const GaDesc& gd, int64_t N, float* genes_out, cudaStream_t st) {
+cudaError_t launch_ga_init(const GaDesc& gd, int npar, int64_t N, float* genes_out, cudaStream_t st) {
     const int64_t total = N * gd.pop;
-    ga_init_kernel<<<grid_for((total + 255) / 256), 256, 0, st>>>(gd, N, genes_out);
+    if (npar == ME_MAX_NPAR) ga_init_kernel<ME_MAX_NPAR><<<grid_for((total + 255) / 256), 256, 0, st>>>(gd, N, genes_out);
+    else ga_init_kernel<ME_NPAR><<<grid_for((total + 255) / 256), 256, 0, st>>>(gd, N, genes_out);
     return cudaGetLastError();
 }
 

@@ -98,7 +98,11 @@ def test_argument_validation_without_gpu(lib):
     bad = B._GaCfg.from_buffer_copy(cfg); bad.pixel_id_base = 2 ** 32 - 2
     assert call(cfg=bad) == -3
     ld11 = B.line_data_from_workload(c0["lines"], True); ld11.c.n_params = 11
-    assert call(ld=ld11.c) == -4
+    assert call(ld=ld11.c) == -1                               # 11 parameters without the fixed profile (reading F13)
+    ld11.c.n_params = 10
+    assert call(ld=ld11.c) == -2
+    ld9 = B.line_data_from_workload(c0["lines"], True); ld9.c.nm_profile = 16
+    assert call(ld=ld9.c) == -2                                # a fixed profile makes no sense with 9 parameters
     # me_synth
     assert lib.me_synth(one, C.c_int64(0), None, lam_p, C.c_int(lam.size), C.byref(ld.c), one, None, None, None, None) == 0
     assert lib.me_synth(one, C.c_int64(5), None, lam_p, C.c_int(lam.size), C.byref(ld.c), None, None, None, None, None) == -1

@@ -1,0 +1,152 @@
+"""GPU parity of the 11-parameter model (SURVEY.md par. 8(f)-1, BASELINE config 4; reading F13 of DESIGN.md):
+fill fraction alpha (eq. 19) + stray-light fraction s with a fixed unpolarised profile
+(PAPER.md:251), through the C ABI against the oracle.  Same tolerances as the 9-parameter path."""
+import os
+
+import numpy as np
+import pytest
+
+from helpers import oracle_lines
+from oracle import api as orc
+from paper_1208_0302_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+NTHREADS = max(1, (os.cpu_count() or 1))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1208_0302_b200 import binding, build
+    build.build()
+    binding.lib()
+    assert torch.cuda.is_available()
+    return binding
+
+
+def dev(a, dtype=np.float32):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
+
+
+def _setup(B, lines, triplets, lam):
+    ln = oracle_lines(lines, triplets)
+    nm = orc.synth(W.NM_PARAMS[None, :], lam, ln)[0, 0].astype(np.float32)      # I_fixed, rounded once for both sides
+    ld = B.line_data_from_workload(lines, triplets, n_params=11, nm_profile=dev(nm))
+    return ln, nm.astype(np.float64), ld
+
+
+CASES = [("config4 grid, two triplets, L=256", [W.FE_6301, W.FE_6302], True, W.grid(6302.0, 256, 0.012), 700),
+         ("full Zeeman patterns, L=63 (odd)", [W.FE_6301, W.FE_6302], False, W.grid(6302.0, 63, 0.04), 300),
+         ("single triplet L=50", [W.FE_6302], True, W.grid(W.FE_6302["lambda0"], 50, 0.024), 257)]
+
+
+@pytest.mark.parametrize("name,lines,triplets,lam,P", CASES, ids=[c[0] for c in CASES])
+def test_me_synth11_vs_oracle(B, name, lines, triplets, lam, P):
+    ln, nm, ld = _setup(B, lines, triplets, lam)
+    p = W.draw_truth(P, seed=31, b_lo=1.0, b_hi=3000.0, npar=11)
+    p[:4, 9] = [0.0, 1.0, 0.0, 1.0]; p[:4, 10] = [0.0, 0.0, 0.3, 0.3]          # corners of the (alpha, s) box
+    mu = np.random.default_rng(2).uniform(0.05, 1.0, P)
+    ref = orc.synth(p, lam, ln, mu=mu, nm_profile=nm, threads=NTHREADS)
+    out, _ = B.me_synth(dev(p), lam, ld, mu=dev(mu))
+    cont = (p[:, 7] + mu * p[:, 8])[:, None, None]
+    err = np.abs(out.cpu().numpy() - ref) / cont
+    assert err.max() <= 2e-5, (name, err.max(), np.unravel_index(err.argmax(), err.shape))
+    # alpha = 1, s = 0 reproduces the 9-parameter kernel bit for bit in Q, U, V and to rounding in I
+    q = p.copy(); q[:, 9] = 1.0; q[:, 10] = 0.0
+    a11, _ = B.me_synth(dev(q), lam, ld, mu=dev(mu))
+    a9, _ = B.me_synth(dev(q[:, :9]), lam, B.line_data_from_workload(lines, triplets), mu=dev(mu))
+    assert torch.equal(a11[:, 1:], a9[:, 1:])
+    assert float((a11[:, 0] - a9[:, 0]).abs().max()) <= 2e-6
+    # fused chi2 uses nu = 4L - 11
+    obs = ref[0] + W.draw_noise(ref[0].shape, 3e-3)
+    w, sg = np.array([1.0, 4.0, 4.0, 2.0]), np.full(4, 3e-3)
+    want = np.array([orc.chi2(obs, m, w, sg, M=11) for m in ref[:64]])
+    _, chi = B.me_synth(dev(p[:64]), lam, ld, mu=dev(mu[:64]), obs_ref=dev(obs), w_over_sigma=w / sg, want_stokes=False)
+    assert np.max(np.abs(chi.cpu().numpy() - want) / want) < 2e-4
+
+
+@pytest.mark.parametrize("pop,k", [(64, 3), (100, 2), (512, 3)])
+def test_ga_init_and_step_bit_exact_eleven_genes(B, pop, k):
+    cfg = W.ga_config(pop, 12, tournament_k=k, npar=11)
+    N, seed, base = 19, 0x5EED5EED5, 123456
+    g0 = B.ga_init(N, cfg, seed, pixel_id_base=base)
+    assert g0.shape == (N, pop, 11)
+    assert np.array_equal(g0.cpu().numpy(), orc.ga_init(N, pop, seed, pixel_base=base, npar=11))
+    rng = np.random.default_rng(pop)
+    genes = rng.random((N, pop, 11)).astype(np.float32)
+    chi2 = (rng.random((N, pop)) * 50).astype(np.float32)
+    chi2[0, : pop // 2] = chi2[0, 0]
+    for t in (1, 5, 12):
+        got = B.ga_step(dev(genes), dev(chi2), t, cfg, seed, pixel_id_base=base).cpu().numpy()
+        want = orc.ga_step(genes, chi2.astype(np.float64), t, cfg, seed, pixel_base=base)
+        assert np.array_equal(got, want), (pop, k, t)
+
+
+@pytest.mark.parametrize("triplets", [True, False])
+def test_fused_fitness11_vs_oracle(B, triplets):
+    c4 = W.config4()
+    lam = c4["lam"] if triplets else W.grid(6302.0, 101, 0.03)
+    ln, nm, ld = _setup(B, c4["lines"], triplets, lam)
+    N, pop = 6, 96
+    ga = W.ga_config(pop, 5, sigma=3e-3, b_lo=1.0, b_hi=500.0, npar=11)
+    mu = np.linspace(0.2, 1.0, N)
+    truth = W.draw_truth(N, seed=4, b_lo=1.0, b_hi=500.0, npar=11)
+    clean = orc.synth(truth, lam, ln, mu=mu, nm_profile=nm, threads=NTHREADS)
+    obs = (clean + W.draw_noise(clean.shape, 3e-3)).astype(np.float32).astype(np.float64)
+    genes = orc.ga_init(N, pop, seed=12, npar=11)
+    genes[:, 0, :] = 0.0; genes[:, 1, :] = 1.0
+    want = orc.ga_fitness(genes, obs, lam, ln, ga, mu=mu, threads=NTHREADS, nm_profile=nm)
+    got = B.ga_fitness(dev(genes), dev(obs), lam, ld, ga, mu=dev(mu)).cpu().numpy().astype(np.float64)
+    rel = np.abs(got - want) / want
+    assert rel.max() < 2e-4, rel.max()
+    assert np.median(rel) < 1e-5
+
+
+def _errors(params, truth):
+    dchi = np.abs(params[:, 2] - truth[:, 2]) % 180.0
+    return dict(B=np.abs(params[:, 0] - truth[:, 0]), gamma=np.abs(params[:, 1] - truth[:, 1]),
+                chi=np.minimum(dchi, 180.0 - dchi), v=np.abs(params[:, 6] - truth[:, 6]), alpha=np.abs(params[:, 9] - truth[:, 9]))
+
+
+def test_inversion11_statistical_parity(B):
+    # the config-4 model on a size the oracle finishes in about a minute: 64 pixels, L = 64, pop 64, 40 generations
+    lines, lam = [W.FE_6301, W.FE_6302], W.grid(6302.0, 64, 0.048)
+    ln, nm, ld = _setup(B, lines, True, lam)
+    N = 64
+    ga = W.ga_config(64, 40, sigma=3e-3, b_lo=1.0, b_hi=500.0, npar=11)
+    truth = W.draw_truth(N, seed=W.SEED_TRUTH, b_lo=1.0, b_hi=500.0, npar=11)
+    clean = orc.synth(truth, lam, ln, nm_profile=nm, threads=NTHREADS)
+    obs = (clean + W.draw_noise(clean.shape, 3e-3)).astype(np.float32).astype(np.float64)
+    res = orc.ga_invert(obs, lam, ln, ga, seed=W.SEED_GA, nm_profile=nm, threads=NTHREADS)
+    gp, gc = B.ga_invert(dev(obs), lam, ld, ga, W.SEED_GA)
+    gp, gc = gp.cpu().numpy().astype(np.float64), gc.cpu().numpy().astype(np.float64)
+    assert gp.shape == (N, 11)
+    same = np.abs(gc - res["chi2"]) <= 2e-4 * res["chi2"]
+    assert same.mean() >= 0.85, same.mean()
+    assert abs(np.median(gc) - np.median(res["chi2"])) <= 0.01 * np.median(res["chi2"])
+    eg, eo = _errors(gp, truth), _errors(res["params"], truth)
+    for k in eg:
+        a, b = np.median(eg[k]), np.median(eo[k])
+        assert abs(a - b) <= 0.05 * b, (k, a, b)
+    # the returned chi2 is the chi2 of the returned parameters (oracle evaluates the GPU's answer)
+    model = orc.synth(gp, lam, ln, nm_profile=nm, threads=NTHREADS)
+    chk = np.array([orc.chi2(o, m, ga["stokes_weight"], ga["sigma"], M=11) for o, m in zip(obs, model)])
+    assert np.max(np.abs(gc - chk) / chk) < 5e-4
+
+
+def test_config4_launch_configuration_sampled(B):
+    # BASELINE config 4's launch configuration (L = 256, pop 512 -> 512-thread CTAs, 11 genes) with the generation
+    # count cut to 20 so that the oracle can follow 8 pixels; global pixel ids as in a full-map run.
+    c4 = W.config4()
+    ln, nm, ld = _setup(B, c4["lines"], True, c4["lam"])
+    N, base = 8, 200000
+    ga = W.ga_config(512, 20, sigma=3e-3, b_lo=1.0, b_hi=500.0, npar=11)
+    truth = W.draw_truth(N, seed=77, b_lo=1.0, b_hi=500.0, npar=11)
+    clean = orc.synth(truth, c4["lam"], ln, nm_profile=nm, threads=NTHREADS)
+    obs = (clean + W.draw_noise(clean.shape, 3e-3)).astype(np.float32).astype(np.float64)
+    res = orc.ga_invert(obs, c4["lam"], ln, ga, seed=W.SEED_GA, nm_profile=nm, pixel_base=base, threads=NTHREADS)
+    gp, gc = B.ga_invert(dev(obs), c4["lam"], ld, ga, W.SEED_GA, pixel_id_base=base)
+    gc = gc.cpu().numpy().astype(np.float64)
+    same = np.abs(gc - res["chi2"]) <= 2e-4 * res["chi2"]
+    assert same.mean() >= 0.75, (same.mean(), gc, res["chi2"])
+    assert np.all(np.abs(gc - res["chi2"]) <= 0.25 * res["chi2"])
