@@ -3,7 +3,7 @@
 
 A "step" is one pass of the whole hot path over one batch: one `ga_invert` call (observation staging, generation 0,
 G generations of select/crossover/mutate/evaluate, output) over the map of the chosen workload.
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config1|config3|config0] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config1|config3|config4|config0] [--impl reference]
 One JSON line on stdout (rank 0).  See DESIGN.md "Measurement" for every field.
 """
 import argparse
@@ -27,9 +27,9 @@ from paper_1208_0302_b200 import workloads as W  # noqa: E402
 # SASS opcode / lambda-points; FFMA2 = 4 flop, FMUL2 / FADD2 / FFMA = 2, FMUL / FADD = 1).  It is re-counted whenever the
 # kernel changes (r1a: 477, r1b: 280, r1c: 265.7), so `frac` is the FP32-pipe utilisation, not an inflated textbook
 # count.  See DESIGN.md "Measurement".  config0 (one line) is not the bench default and carries an estimate.
-FLOP_PER_POINT = {"config0_tiny": 150.0, "config1_map256": 265.7, "config3_fulldisc": 265.7}
+FLOP_PER_POINT = {"config0_tiny": 150.0, "config1_map256": 265.7, "config3_fulldisc": 265.7, "config4_stress11": 266.3}
 # DRAM traffic of ga_invert_kernel per pixel, from the same capture (dram__bytes_read.sum + write.sum) / pixels
-DRAM_BYTES_PER_PIXEL_NCU = 8.878848e6 / 4096
+DRAM_BYTES_PER_PIXEL_NCU = 8.878848e6 / 4096      # at L = 128 (2088 algorithmic bytes); scaled by 16 L + 40 for other grids
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 
 
@@ -38,8 +38,8 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config3"])
-    ap.add_argument("--n-side", type=int, default=0, help="override the map side (config1: 256, config3: 2048)")
+    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config3", "config4"])
+    ap.add_argument("--n-side", type=int, default=0, help="override the map side (config1: 256, config3: 2048, config4: 512)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -54,6 +54,10 @@ def workload(args):
     if args.workload == "config1":
         side = args.n_side or 256
         c = W.config1(side)
+        return c, side * side, None
+    if args.workload == "config4":
+        side = args.n_side or 512
+        c = W.config4(side)
         return c, side * side, None
     side = args.n_side or 2048
     c = W.config3(side)
@@ -122,18 +126,36 @@ def oracle_sample(cfg, n, stream=0):
     """n pixels of the workload, observations synthesised by the oracle itself (+ seeded noise, rounded to f32)."""
     from oracle import api as orc
     ln = oracle_lines_for(cfg)
-    truth = W.draw_truth(n, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=100 + stream)
-    clean = orc.synth(truth, cfg["lam"], ln, threads=orc.hardware_threads())
+    npar = cfg.get("npar", 9)
+    truth = W.draw_truth(n, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=100 + stream, npar=npar)
+    nm = orc.synth(W.NM_PARAMS[None, :], cfg["lam"], ln)[0, 0] if npar == 11 else None
+    clean = orc.synth(truth, cfg["lam"], ln, threads=orc.hardware_threads(), nm_profile=nm)
     obs = (clean + W.draw_noise(clean.shape, cfg["sigma"], stream=100 + stream)).astype(np.float32).astype(np.float64)
-    return ln, obs
+    return ln, obs, nm
+
+
+def bounded_oracle_cfg(cfg, core_seconds_per_pixel=12.0):
+    """The oracle needs ~2 us per wavelength point per core (x2 for the 11-parameter model).  Where one pixel of the
+    workload would take much longer than the budget (config4: ~150 core-s), the sample runs the SAME pixel problem for
+    fewer generations and the result is reported in pixel-equivalents: pixels x (syntheses done / syntheses of a full
+    inversion).  Returns (cfg for the oracle, that fraction, a note for the sample text)."""
+    ga = cfg["ga"]
+    per_synth = 2.0e-6 * cfg["lam"].size * (2 if cfg.get("npar", 9) == 11 else 1) * len(cfg["lines"]) / 2.0
+    full = syntheses_per_pixel(ga)
+    if full * per_synth <= 2.5 * core_seconds_per_pixel:
+        return cfg, 1.0, ""
+    g = max(1, int((core_seconds_per_pixel / per_synth - ga["pop"]) / (ga["pop"] - 1)))
+    ga2 = dict(ga, generations=g, mut_scale=ga["mut_scale"][:g + 1])
+    frac = (ga["pop"] + g * (ga["pop"] - 1)) / full
+    return dict(cfg, ga=ga2), frac, " cut to %d of %d generations (value in pixel-equivalents by syntheses)" % (g, ga["generations"])
 
 
 def time_oracle(cfg, n, stream=0):
     from oracle import api as orc
-    ln, obs = oracle_sample(cfg, n, stream)
+    ln, obs, nm = oracle_sample(cfg, n, stream)
     cores = orc.hardware_threads()
     t0 = time.perf_counter()
-    orc.ga_invert(obs, cfg["lam"], ln, cfg["ga"], seed=W.SEED_GA, threads=cores)
+    orc.ga_invert(obs, cfg["lam"], ln, cfg["ga"], seed=W.SEED_GA, threads=cores, nm_profile=nm)
     return time.perf_counter() - t0, cores
 
 
@@ -145,17 +167,18 @@ def run_reference(args):
     from oracle import api as orc
     cfg, n_pixels, _ = workload(args)
     cores = orc.hardware_threads()
-    per_pixel_points = syntheses_per_pixel(cfg["ga"]) * cfg["lam"].size * sum(3 for _ in cfg["lines"])
+    ocfg, frac, note = bounded_oracle_cfg(cfg, core_seconds_per_pixel=6.0)
+    per_pixel_points = syntheses_per_pixel(ocfg["ga"]) * cfg["lam"].size * sum(3 for _ in cfg["lines"])
     n = max(cores, int(cores * max(1.0, 2.0e7 / per_pixel_points)))      # ~ a few seconds of work per core per step
     n = min(n, n_pixels)
     for w in range(args.warmup):
-        time_oracle(cfg, n, stream=w)
+        time_oracle(ocfg, n, stream=w)
     t = 0.0
     for k in range(args.steps):
-        dt, _ = time_oracle(cfg, n, stream=args.warmup + k)
+        dt, _ = time_oracle(ocfg, n, stream=args.warmup + k)
         t += dt
-    val = n * args.steps / t
-    sample = "%d pixels of %s per step (oracle-synthesised obs), all %d host threads" % (n, cfg["name"], cores)
+    val = n * frac * args.steps / t
+    sample = "%d pixels of %s%s per step (oracle-synthesised obs), all %d host threads" % (n, cfg["name"], note, cores)
     line = {"impl": "reference", "metric": "pixel-inversions/s", "value": val, "unit": "pixels/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -172,8 +195,9 @@ def run_reference(args):
 def build_inputs(cfg, n_pixels, side, rank, torch, B):
     """Synthetic observation cube resident in HBM: truth -> me_synth (this library) -> + Gaussian noise (device RNG)."""
     dev = torch.device("cuda")
+    npar = cfg.get("npar", 9)
     if side is None:
-        truth = W.draw_truth(n_pixels, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=rank)
+        truth = W.draw_truth(n_pixels, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=rank, npar=npar)
         mask_t = mu_t = None
         n_active = n_pixels
     else:
@@ -182,6 +206,9 @@ def build_inputs(cfg, n_pixels, side, rank, torch, B):
         mu_t = torch.from_numpy(mu.astype(np.float32)).to(dev)
         n_active = int(mask.sum())
     ld = B.line_data_from_workload(cfg["lines"], cfg["triplets"])
+    if npar == 11:        # reading F13: I_fixed = the B = 0 profile of workloads.NM_PARAMS, synthesised by this library
+        nm, _ = B.me_synth(torch.from_numpy(W.NM_PARAMS[None, :].astype(np.float32)).to(dev), cfg["lam"], ld)
+        ld = B.line_data_from_workload(cfg["lines"], cfg["triplets"], n_params=11, nm_profile=nm[0, 0].contiguous())
     truth_t = torch.from_numpy(truth.astype(np.float32)).to(dev)
     obs, _ = B.me_synth(truth_t, cfg["lam"], ld, mu=mu_t)
     gen = torch.Generator(device=dev)
@@ -248,7 +275,7 @@ def run_b200(args):
     ld, obs, mask_t, mu_t, n_active, _ = build_inputs(cfg, n_pixels, side, rank, torch, B)
     ga, lam = cfg["ga"], cfg["lam"]
     base = rank * n_pixels                                    # shards keyed by global pixel id (no data-path collective)
-    out_p = torch.empty((n_pixels, 9), dtype=torch.float32, device="cuda")
+    out_p = torch.empty((n_pixels, cfg.get("npar", 9)), dtype=torch.float32, device="cuda")
     out_c = torch.empty((n_pixels,), dtype=torch.float32, device="cuda")
 
     def step():
@@ -335,7 +362,7 @@ def run_b200(args):
                        "l2": "obs cube %.0f MB per step (> 126 MB L2 for config1/3); path is ALU-bound" % (obs.numel() * 4 / 1e6)},
             "syntheses_per_s": value * syn, "median_chi2": med_chi2,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": DRAM_BYTES_PER_PIXEL_NCU * n_active, "algorithmic_bytes": (16 * L + 40) * n_active,
+                         "traffic": DRAM_BYTES_PER_PIXEL_NCU * n_active * (16 * L + 40) / 2088.0, "algorithmic_bytes": (16 * L + 40) * n_active,
                          "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt,
                          "peak_measured_ffma_tflops": probe["ffma"]["tflops"],
                          "mufu_per_s_measured": probe["mufu"]["thread_inst_per_s"],
@@ -347,10 +374,11 @@ def run_b200(args):
     if not args.no_cpu_baseline:
         from oracle import api as orc
         cores = orc.hardware_threads()
-        n = min(n_pixels, 2 * cores)
-        dt, cores = time_oracle(cfg, n)
-        line["cpu_baseline"] = {"value": n / dt, "unit": "pixels/s", "cores": cores, "kind": "oracle",
-                                "sample": "%d pixels of %s, oracle-synthesised obs, %.1f s" % (n, cfg["name"], dt)}
+        ocfg, frac, note = bounded_oracle_cfg(cfg)
+        n = min(n_pixels, (2 if frac == 1.0 else 1) * cores)
+        dt, cores = time_oracle(ocfg, n)
+        line["cpu_baseline"] = {"value": n * frac / dt, "unit": "pixels/s", "cores": cores, "kind": "oracle",
+                                "sample": "%d pixels of %s%s, oracle-synthesised obs, %.1f s" % (n, cfg["name"], note, dt)}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
