@@ -89,6 +89,17 @@ def _npar(cfg):
     return int(len(cfg["lo"]))
 
 
+def _variant(cfg):
+    """0 = real-coded operators (readings G1-G3), 1 = the paper's binary-coded GA (readings V0-V5)."""
+    return int(cfg.get("variant", 0))
+
+
+def sobol(n0, count, dims):
+    out = np.zeros((count, dims), dtype=np.uint32)
+    lib().orc_sobol(C.c_uint32(n0), C.c_int(count), C.c_int(dims), _p(out, C.c_uint32))
+    return out
+
+
 def _nm(nm_profile, npar, L):
     if npar == NPAR:
         return None
@@ -146,13 +157,13 @@ def decode(genes, cfg):
     genes = np.ascontiguousarray(genes, dtype=np.float32).reshape(-1, npar)
     out = np.empty(genes.shape)
     lo, hi, lg = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"])
-    lib().orc_decode(_p(genes, C.c_float), C.c_int(npar), C.c_int64(genes.shape[0]), _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(out, C.c_double))
+    lib().orc_decode(_p(genes, C.c_float), C.c_int(npar), C.c_int(_variant(cfg)), C.c_int64(genes.shape[0]), _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(out, C.c_double))
     return out
 
 
-def ga_init(N, pop, seed, pixel_base=0, npar=NPAR):
+def ga_init(N, pop, seed, pixel_base=0, npar=NPAR, variant=0):
     genes = np.empty((N, pop, npar), dtype=np.float32)
-    lib().orc_ga_init(C.c_int64(N), C.c_uint64(pixel_base), C.c_int(pop), C.c_int(npar), C.c_uint64(seed), _p(genes, C.c_float))
+    lib().orc_ga_init(C.c_int64(N), C.c_uint64(pixel_base), C.c_int(pop), C.c_int(npar), C.c_int(variant), C.c_uint64(seed), _p(genes, C.c_float))
     return genes
 
 
@@ -172,7 +183,7 @@ def ga_step(genes, chi2v, t, cfg, seed, pixel_base=0):
     keep, a = _cfg_args(cfg)
     per = _i32(cfg["periodic"])
     lib().orc_ga_step(_p(genes, C.c_float), _p(chi2v, C.c_double), C.c_int64(N), C.c_uint64(pixel_base), C.c_int(t),
-                      *a, _p(per, C.c_int), C.c_int(genes.shape[2]), C.c_uint64(seed), _p(out, C.c_float))
+                      *a, _p(per, C.c_int), C.c_int(genes.shape[2]), C.c_int(_variant(cfg)), C.c_uint64(seed), _p(out, C.c_float))
     return out
 
 
@@ -190,7 +201,7 @@ def ga_fitness(genes, obs, lam, lines, cfg, mu=None, threads=1, nm_profile=None)
     lib().orc_ga_fitness(_p(genes, C.c_float), _p(obs, C.c_double), _p(mu_a, C.c_double), C.c_int64(N), C.c_int(pop),
                          _p(lam, C.c_double), C.c_int(lam.size), *lines.args(),
                          _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(w, C.c_double), _p(sg, C.c_double),
-                         C.c_int(npar), _p(nm, C.c_double), C.c_int(threads), _p(out, C.c_double))
+                         C.c_int(npar), C.c_int(_variant(cfg)), _p(nm, C.c_double), C.c_int(threads), _p(out, C.c_double))
     return out
 
 
@@ -212,6 +223,6 @@ def ga_invert(obs, lam, lines, cfg, seed, mask=None, mu=None, pixel_base=0, thre
     lib().orc_ga_invert(_p(obs, C.c_double), _p(mask_a, C.c_ubyte), _p(mu_a, C.c_double), C.c_int64(N), C.c_uint64(pixel_base),
                         _p(lam, C.c_double), C.c_int(L), *lines.args(), *a,
                         _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(per, C.c_int),
-                        _p(w, C.c_double), _p(sg, C.c_double), C.c_int(npar), _p(nm, C.c_double), C.c_uint64(seed), C.c_int(threads),
+                        _p(w, C.c_double), _p(sg, C.c_double), C.c_int(npar), C.c_int(_variant(cfg)), _p(nm, C.c_double), C.c_uint64(seed), C.c_int(threads),
                         _p(params, C.c_double), _p(chi2v, C.c_double), _p(genes, C.c_float), _p(trace, C.c_double))
     return {"params": params, "chi2": chi2v, "genes": genes, "trace": trace}

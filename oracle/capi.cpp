@@ -35,8 +35,8 @@ template <class F> void parallel_for(int64_t n, int threads, F f) {
 
 GaCfg make_cfg(int pop, int generations, int tournament_k, float p_cross, float p_mut, const float* mut_scale,
                const double* lo, const double* hi, const int* log_scale, const int* periodic,
-               const double* w, const double* sigma, uint64_t seed, int npar = NPAR, const double* nm_profile = nullptr) {
-    GaCfg c; c.npar = npar; c.nm_profile = nm_profile; c.pop = pop; c.generations = generations; c.tournament_k = tournament_k;
+               const double* w, const double* sigma, uint64_t seed, int npar = NPAR, const double* nm_profile = nullptr, int variant = 0) {
+    GaCfg c; c.variant = variant; c.npar = npar; c.nm_profile = nm_profile; c.pop = pop; c.generations = generations; c.tournament_k = tournament_k;
     c.p_cross = p_cross; c.p_mut = p_mut; c.mut_scale.assign(mut_scale, mut_scale + generations + 1);
     for (int j = 0; j < npar; ++j) { c.lo[j] = lo[j]; c.hi[j] = hi[j]; c.log_scale[j] = log_scale[j]; c.periodic[j] = periodic[j]; }
     for (int s = 0; s < 4; ++s) { c.w[s] = w[s]; c.sigma[s] = sigma[s]; }
@@ -94,24 +94,30 @@ void orc_philox(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c
     uint32_t ctr[4] = { c0, c1, c2, c3 }, key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
     philox4x32_10(ctr, key, out);
 }
+// count Sobol' points starting at index n0, dims dimensions: out[count][dims] (32-bit fixed point).
+void orc_sobol(uint32_t n0, int count, int dims, uint32_t* out) {
+    for (int i = 0; i < count; ++i)
+        for (int j = 0; j < dims; ++j) out[i * dims + j] = sobol_point(n0 + (uint32_t)i, j);
+}
 void orc_philox_raw(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
 
-void orc_decode(const float* genes, int npar, int64_t n, const double* lo, const double* hi, const int* log_scale, double* out) {
+void orc_decode(const float* genes, int npar, int variant, int64_t n, const double* lo, const double* hi, const int* log_scale, double* out) {
+    GaCfg c; c.variant = variant;
     for (int64_t i = 0; i < n; ++i)
-        for (int j = 0; j < npar; ++j) out[i * npar + j] = decode_gene(genes[i * npar + j], lo[j], hi[j], log_scale[j]);
+        for (int j = 0; j < npar; ++j) out[i * npar + j] = decode_gene(gene_value(genes[i * npar + j], c), lo[j], hi[j], log_scale[j]);
 }
 
-void orc_ga_init(int64_t N, uint64_t pixel_base, int pop, int npar, uint64_t seed, float* genes) {
-    GaCfg c; c.pop = pop; c.seed = seed; c.npar = npar;
+void orc_ga_init(int64_t N, uint64_t pixel_base, int pop, int npar, int variant, uint64_t seed, float* genes) {
+    GaCfg c; c.pop = pop; c.seed = seed; c.npar = npar; c.variant = variant;
     for (int64_t n = 0; n < N; ++n) ga_init(pixel_base + n, c, genes + n * pop * npar);
 }
 
 // One generation for N pixels: genes_in[N][pop][9], chi2_in[N][pop] (double) -> genes_out.
 void orc_ga_step(const float* genes_in, const double* chi2_in, int64_t N, uint64_t pixel_base, int t,
                  int pop, int generations, int tournament_k, float p_cross, float p_mut, const float* mut_scale,
-                 const int* periodic, int npar, uint64_t seed, float* genes_out) {
+                 const int* periodic, int npar, int variant, uint64_t seed, float* genes_out) {
     double z[MAXPAR] = {0}; int zi[MAXPAR] = {0}; double w4[4] = {1, 1, 1, 1};
-    GaCfg c = make_cfg(pop, generations, tournament_k, p_cross, p_mut, mut_scale, z, z, zi, periodic, w4, w4, seed, npar);
+    GaCfg c = make_cfg(pop, generations, tournament_k, p_cross, p_mut, mut_scale, z, z, zi, periodic, w4, w4, seed, npar, nullptr, variant);
     for (int64_t n = 0; n < N; ++n)
         ga_step(genes_in + n * pop * npar, chi2_in + n * pop, t, pixel_base + n, c, genes_out + n * pop * npar);
 }
@@ -121,12 +127,13 @@ void orc_ga_fitness(const float* genes, const double* obs, const double* mu, int
                     int n_lines, const double* lambda0, const double* strength, const int* n_comp,
                     const double* shift, const double* weight, const int* kind, double lambda_ref,
                     const double* lo, const double* hi, const int* log_scale, const double* w, const double* sigma,
-                    int npar, const double* nm_profile, int threads, double* chi2_out) {
+                    int npar, int variant, const double* nm_profile, int threads, double* chi2_out) {
+    GaCfg gv; gv.variant = variant;
     Lines ln = make_lines(n_lines, lambda0, strength, n_comp, shift, weight, kind, lambda_ref);
     parallel_for(N * pop, threads, [&](int64_t k) {
         int64_t n = k / pop;
         double p[MAXPAR];
-        for (int j = 0; j < npar; ++j) p[j] = decode_gene(genes[k * npar + j], lo[j], hi[j], log_scale[j]);
+        for (int j = 0; j < npar; ++j) p[j] = decode_gene(gene_value(genes[k * npar + j], gv), lo[j], hi[j], log_scale[j]);
         std::vector<double> model(4 * L);
         synth_n(p, npar, mu ? mu[n] : 1.0, lambda, L, ln, nm_profile, model.data(), false);
         double x = chi2(obs + n * 4 * L, model.data(), L, w, sigma, npar);
@@ -141,10 +148,10 @@ void orc_ga_invert(const double* obs, const unsigned char* mask, const double* m
                    const double* shift, const double* weight, const int* kind, double lambda_ref,
                    int pop, int generations, int tournament_k, float p_cross, float p_mut, const float* mut_scale,
                    const double* lo, const double* hi, const int* log_scale, const int* periodic,
-                   const double* w, const double* sigma, int npar, const double* nm_profile, uint64_t seed, int threads,
+                   const double* w, const double* sigma, int npar, int variant, const double* nm_profile, uint64_t seed, int threads,
                    double* out_params, double* out_chi2, float* out_genes, double* trace) {
     Lines ln = make_lines(n_lines, lambda0, strength, n_comp, shift, weight, kind, lambda_ref);
-    GaCfg c = make_cfg(pop, generations, tournament_k, p_cross, p_mut, mut_scale, lo, hi, log_scale, periodic, w, sigma, seed, npar, nm_profile);
+    GaCfg c = make_cfg(pop, generations, tournament_k, p_cross, p_mut, mut_scale, lo, hi, log_scale, periodic, w, sigma, seed, npar, nm_profile, variant);
     parallel_for(N, threads, [&](int64_t n) {
         if (mask && !mask[n]) {
             for (int j = 0; j < npar; ++j) out_params[n * npar + j] = std::nan("");

@@ -10,7 +10,9 @@
 // the fitness is double here.
 #include "oracle.hpp"
 #include <cmath>
+#include <algorithm>
 #include <limits>
+#include <vector>
 
 namespace orc {
 
@@ -25,14 +27,98 @@ static void draw(const GaCfg& c, uint64_t pixel, int t, int i, int k, uint32_t o
     philox4x32_10(ctr, key, out);
 }
 
+// V0 / eq. 5: a 16-bit code k decodes to g = k / (2^N - 1); the real-coded variant holds g itself.  The result is
+// rounded to binary32 so that both implementations feed the same gene value to the box mapping.
+float gene_value(float stored, const GaCfg& c) { return c.variant == 1 ? stored / 65535.0f : stored; }   // one IEEE binary32 division
+
 // G1: gene in [0,1] -> physical parameter, from the binary32 gene, in double.
 double decode_gene(float g, double lo, double hi, int log_scale) {
     if (log_scale) return lo * std::pow(hi / lo, (double)g);
     return lo + (hi - lo) * (double)g;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Variant 1: the paper's own binary-coded GA (readings V0-V5 of DESIGN.md).
+//   V0  genotype: one 16-bit unsigned code k per parameter, held here as an integer-valued float;
+//       decode (eq. 5): g = k / (2^16 - 1), then the box mapping of reading G1.
+//   V1  initial population: individual i = Sobol' point number i + 1 in M dimensions, top 16 bits per
+//       dimension, xor a per-pixel digital shift (16 bits per dimension from Philox block (pixel, 0, 2^32-1, j/4)).
+//   V2  restart: every N_samp = max(1, G/4) generations (t mod N_samp = 0, t < G) the worst floor(P/2)
+//       members of generation t-1 (rank by chi2, ties by index) are dead: tournaments draw among the live ranks only
+//       and the last floor(P/2) slots of generation t are the NEXT Sobol' points of the same shifted sequence.
+//   V3  selection: the k-way tournament of reading G3.
+//   V4  recombination: children come in pairs (2q-1, 2q) keyed by the odd index; parents A, B from
+//       blocks 0, 1; block 2: u0 < p_cross ? one-point crossover at bit cut = 1 + floor(u1 (16 M - 1)) of the M x 16
+//       bit string (gene 0 first, bit 0 = MSB) : copies; the odd child takes head(A) + tail(B), the even
+//       child head(B) + tail(A).
+//   V5  mutation ("less-significant bits more frequently"): gene j of child i, words (x_m, x_d) of
+//       block 3 + j/2: if u(x_m) < p_mut flip the bits of ((x_d & 0xffff) & (x_d >> 16)) >> (x_m & 15), so that bit b
+//       (0 = LSB) flips with probability (16 - b) / 64.
+// ---------------------------------------------------------------------------------------------------------
+static uint32_t digital_shift(const GaCfg& c, uint64_t pixel, int j) {
+    uint32_t r[4];
+    draw(c, pixel, 0, (int)0xFFFFFFFFu, j / 4, r);
+    return r[j % 4] >> 16;
+}
+
+static float sobol_gene(const GaCfg& c, uint64_t pixel, uint32_t n, int j) {
+    return (float)(((sobol_point(n, j) >> 16) ^ digital_shift(c, pixel, j)) & 0xFFFFu);
+}
+
+static void ga_init_binary(uint64_t pixel, const GaCfg& c, float* genes) {
+    for (int i = 0; i < c.pop; ++i)
+        for (int j = 0; j < c.npar; ++j) genes[i * c.npar + j] = sobol_gene(c, pixel, (uint32_t)i + 1u, j);
+}
+
+static void ga_step_binary(const float* genes, const double* chi2v, int t, uint64_t pixel, const GaCfg& c, float* out) {
+    const int M = c.npar, P = c.pop;
+    const int n_samp = c.generations / 4 > 1 ? c.generations / 4 : 1;
+    const bool restart = (t % n_samp == 0) && t < c.generations;
+    const int n_dead = restart ? P / 2 : 0, n_live = P - n_dead;
+    std::vector<int> order(P);                                           // order[r] = index of the r-th best
+    for (int i = 0; i < P; ++i) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return chi2v[a] < chi2v[b]; });
+    for (int j = 0; j < M; ++j) out[j] = genes[order[0] * M + j];        // elite (ties -> lowest index)
+    auto pick = [&](const uint32_t r[4]) {
+        int best = order[below(r[0], n_live)];
+        for (int m = 1; m < c.tournament_k; ++m) {
+            int cand = order[below(r[m], n_live)];
+            if (chi2v[cand] < chi2v[best] || (chi2v[cand] == chi2v[best] && cand < best)) best = cand;
+        }
+        return best;
+    };
+    for (int i = 1; i < P; ++i) {
+        if (i >= n_live) {                                               // V2: fresh points
+            const uint32_t n = (uint32_t)(P + (t / n_samp - 1) * n_dead + (i - n_live) + 1);
+            for (int j = 0; j < M; ++j) out[i * M + j] = sobol_gene(c, pixel, n, j);
+            continue;
+        }
+        const int key = 2 * ((i + 1) / 2) - 1;                           // V4: pair (2q-1, 2q) keyed by 2q-1
+        uint32_t r[4];
+        draw(c, pixel, t, key, 0, r);  const int A = pick(r);
+        draw(c, pixel, t, key, 1, r);  const int B = pick(r);
+        draw(c, pixel, t, key, 2, r);
+        const bool cross = u01(r[0]) < c.p_cross;
+        const int cut = 1 + below(r[1], 16 * M - 1);
+        const int first = (i & 1) ? A : B, second = (i & 1) ? B : A;
+        for (int j = 0; j < M; ++j) {
+            uint32_t k1 = (uint32_t)genes[first * M + j], k2 = (uint32_t)genes[second * M + j], k = k1;
+            if (cross) {
+                int nhead = cut - 16 * j; nhead = nhead < 0 ? 0 : (nhead > 16 ? 16 : nhead);
+                const uint32_t mask = (0xFFFFu << (16 - nhead)) & 0xFFFFu;
+                k = (k1 & mask) | (k2 & ~mask & 0xFFFFu);
+            }
+            if (j % 2 == 0) draw(c, pixel, t, i, 3 + j / 2, r);          // V5: own draws of child i
+            const uint32_t xm = r[2 * (j % 2)], xd = r[2 * (j % 2) + 1];
+            if (u01(xm) < c.p_mut) k ^= ((xd & 0xFFFFu) & (xd >> 16)) >> (xm & 15u);
+            out[i * M + j] = (float)k;
+        }
+    }
+}
+
 // G2: generation 0, gene j of individual i = lane (j mod 4) of block floor(j / 4).
 void ga_init(uint64_t pixel, const GaCfg& c, float* genes) {
+    if (c.variant == 1) { ga_init_binary(pixel, c, genes); return; }
     for (int i = 0; i < c.pop; ++i)
         for (int j = 0; j < c.npar; ++j) {
             uint32_t r[4];
@@ -58,6 +144,7 @@ static int tournament(const uint32_t r[4], const double* chi2v, const GaCfg& c) 
 }
 
 void ga_step(const float* genes, const double* chi2v, int t, uint64_t pixel, const GaCfg& c, float* out) {
+    if (c.variant == 1) { ga_step_binary(genes, chi2v, t, pixel, c, out); return; }
     const int M = c.npar;
     const int elite = argmin(chi2v, c.pop);
     for (int j = 0; j < M; ++j) out[j] = genes[elite * M + j];               // slot 0 <- elite of t-1
@@ -86,7 +173,7 @@ void ga_step(const float* genes, const double* chi2v, int t, uint64_t pixel, con
 static double fitness(const float* g, const double* obs, double mu, const double* lambda, int L,
                       const Lines& ln, const GaCfg& c, std::vector<double>& model) {
     double p[MAXPAR];
-    for (int j = 0; j < c.npar; ++j) p[j] = decode_gene(g[j], c.lo[j], c.hi[j], c.log_scale[j]);
+    for (int j = 0; j < c.npar; ++j) p[j] = decode_gene(gene_value(g[j], c), c.lo[j], c.hi[j], c.log_scale[j]);
     synth_n(p, c.npar, mu, lambda, L, ln, c.nm_profile, model.data(), false);
     double x = chi2(obs, model.data(), L, c.w, c.sigma, c.npar);                     // nu = 4L - M
     if (!std::isfinite(x)) x = std::numeric_limits<double>::infinity();              // G4
@@ -111,7 +198,7 @@ void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, 
     }
     const int b = argmin(f.data(), c.pop);                                             // G5
     for (int j = 0; j < M; ++j) {
-        best_params[j] = decode_gene(genes[b * M + j], c.lo[j], c.hi[j], c.log_scale[j]);
+        best_params[j] = decode_gene(gene_value(genes[b * M + j], c), c.lo[j], c.hi[j], c.log_scale[j]);
         if (best_genes) best_genes[j] = genes[b * M + j];
     }
     *best_chi2 = f[b];

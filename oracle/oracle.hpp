@@ -73,12 +73,19 @@ double chi2(const double* obs, const double* model, int L, const double w[4], co
 // ---- Philox4x32-10 (Salmon et al. 2011), reading G0 ----
 void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 
+// ---- Sobol' sequence (Bratley & Fox 1988), dims 0..10 ----
+void sobol_directions(int dim, uint32_t v[32]);
+uint32_t sobol_point(uint32_t n, int dim);      // 32-bit fixed point, Gray-code order, n = 0 is the origin
+
 // ---- GA (Alg. 1; readings G0-G5) ----
 struct GaCfg {
     int pop, generations, tournament_k;
     float p_cross, p_mut;
     std::vector<float> mut_scale;              // s_t for t = 0..generations (built by the caller, binary32)
     int npar = NPAR;                           // 9 or 11 genes
+    int variant = 0;                           // 0: real-coded operators (north_star, readings G1-G3)
+                                               // 1: the paper's binary-coded GA (16-bit genotype, one-point crossover,
+                                               //    LSB-biased bit mutation, Sobol init + restarts; readings V0-V5)
     const double* nm_profile = nullptr;        // I_fixed[L] for npar = 11
     double lo[MAXPAR], hi[MAXPAR];
     int log_scale[MAXPAR], periodic[MAXPAR];
@@ -86,6 +93,7 @@ struct GaCfg {
     uint64_t seed;
 };
 double decode_gene(float g, double lo, double hi, int log_scale);
+float gene_value(float stored, const GaCfg& c);   // variant 1: 16-bit code -> g = k / 65535 (eq. 5), rounded to binary32
 // Next generation from (genes[pop][NPAR], chi2[pop]) at generation t >= 1 for global pixel id `pixel`.
 void ga_step(const float* genes, const double* chi2v, int t, uint64_t pixel, const GaCfg& c, float* out);
 void ga_init(uint64_t pixel, const GaCfg& c, float* genes);
