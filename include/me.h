@@ -100,6 +100,14 @@ typedef struct {
     float stokes_weight[4];   /* w_s of eq. 16 (1,4,4,2 in the configs); enters squared */
     const float* mu;          /* device [N] f32 or NULL (=> 1): cosine of the heliocentric angle per pixel */
     int64_t pixel_id_base;    /* added to the pixel index in the RNG key so that shards reproduce the full run */
+    int variant;              /* 0: real-coded operators above (tournament, arithmetic crossover, bounded mutation);
+                                 1: the paper's own binary-coded GA (readings V0-V5): 16-bit genotype per
+                                    parameter decoded by eq. 5, one-point crossover of the
+                                    M x 16 bit string, bit mutation favouring less-significant bits
+                                    (PAPER.md:103-105), Sobol' initial population and re-seeding of the worst half
+                                    every max(1, G/4) generations. mut_scale* are ignored.
+                                    In the test hooks a gene then holds its code k in [0, 65535] as a float. */
+    int reserved;             /* must be 0 */
 } ga_cfg;
 
 /* GA inversion of N pixels.

@@ -79,10 +79,13 @@ static void ga_step_binary(const float* genes, const double* chi2v, int t, uint6
     for (int i = 0; i < P; ++i) order[i] = i;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return chi2v[a] < chi2v[b]; });
     for (int j = 0; j < M; ++j) out[j] = genes[order[0] * M + j];        // elite (ties -> lowest index)
+    // V3: candidates are member indices exactly as in G3; only at a restart generation (V2) are they drawn among the
+    // live RANKS and mapped through order[].
+    auto member = [&](uint32_t x) { return restart ? order[below(x, n_live)] : below(x, P); };
     auto pick = [&](const uint32_t r[4]) {
-        int best = order[below(r[0], n_live)];
+        int best = member(r[0]);
         for (int m = 1; m < c.tournament_k; ++m) {
-            int cand = order[below(r[m], n_live)];
+            int cand = member(r[m]);
             if (chi2v[cand] < chi2v[best] || (chi2v[cand] == chi2v[best] && cand < best)) best = cand;
         }
         return best;

@@ -45,7 +45,8 @@ class _GaCfg(C.Structure):
                 ("mut_scale_table", C.POINTER(C.c_float)),
                 ("lo", C.c_float * MAX_NPAR), ("hi", C.c_float * MAX_NPAR),
                 ("log_scale", C.c_uint8 * MAX_NPAR), ("periodic", C.c_uint8 * MAX_NPAR),
-                ("stokes_weight", C.c_float * 4), ("mu", C.c_void_p), ("pixel_id_base", C.c_int64)]
+                ("stokes_weight", C.c_float * 4), ("mu", C.c_void_p), ("pixel_id_base", C.c_int64),
+                ("variant", C.c_int), ("reserved", C.c_int)]
 
 
 def lib():
@@ -149,6 +150,8 @@ def make_ga_cfg(cfg, mu=None, pixel_id_base=0):
     import torch
     c.mu = _dev(mu, torch.float32, "mu").value if mu is not None else None
     c.pixel_id_base = int(pixel_id_base)
+    c.variant = int(cfg.get("variant", 0))
+    c.reserved = 0
     return c, (ms, mu)
 
 

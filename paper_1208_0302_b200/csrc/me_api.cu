@@ -63,6 +63,28 @@ int build_synth_desc(const double* lambda, int L, const me_line_data* ld, me::Sy
     return ME_OK;
 }
 
+// Sobol' direction numbers v_1..v_16 (as 32-bit fixed point) of dimension `dim` (0-based), Bratley & Fox (1988) /
+// Antonov & Saleev recurrence on a primitive polynomial of degree s with coefficient bits a and initial values m_1..m_s
+// (Joe & Kuo's table for the first 11 dimensions; reading V1).  m_i = xor_k 2^k a_k m_(i-k) xor 2^s m_(i-s) xor m_(i-s).
+void sobol_directions16(int dim, uint32_t v[16]) {
+    static const int S[11] = {0, 1, 2, 3, 3, 4, 4, 5, 5, 5, 5};
+    static const unsigned A[11] = {0, 0, 1, 1, 2, 1, 4, 2, 4, 7, 11};
+    static const unsigned M0[11][5] = {{0, 0, 0, 0, 0}, {1, 0, 0, 0, 0}, {1, 3, 0, 0, 0}, {1, 3, 1, 0, 0}, {1, 1, 1, 0, 0},
+                                       {1, 1, 3, 3, 0}, {1, 3, 5, 13, 0}, {1, 1, 5, 5, 17}, {1, 1, 5, 5, 5},
+                                       {1, 1, 7, 11, 19}, {1, 1, 5, 1, 1}};
+    uint32_t m[17];
+    const int s = S[dim];
+    for (int i = 1; i <= 16; ++i) {
+        if (dim == 0) { m[i] = 1; continue; }                 // van der Corput
+        if (i <= s) { m[i] = M0[dim][i - 1]; continue; }
+        uint32_t x = m[i - s] ^ (m[i - s] << s);
+        for (int k = 1; k < s; ++k)
+            if ((A[dim] >> (s - 1 - k)) & 1u) x ^= m[i - k] << k;
+        m[i] = x;
+    }
+    for (int i = 1; i <= 16; ++i) v[i - 1] = m[i] << (32 - i);
+}
+
 int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t seed, int64_t N, bool need_sigma,
                   me::GaDesc& g) {
     if (c == nullptr) return ME_ERR_NULL;
@@ -72,6 +94,8 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
     if (c->generations < 0 || c->generations > ME_MAX_GEN) return ME_ERR_SHAPE;
     if (c->tournament_k < 1 || c->tournament_k > 4) return ME_ERR_RANGE;
     if (c->elite != 1) return ME_ERR_UNSUPPORTED;
+    if (c->variant != 0 && c->variant != 1) return ME_ERR_RANGE;
+    if (c->reserved != 0) return ME_ERR_RANGE;
     if (!(c->p_cross >= 0.f && c->p_cross <= 1.f) || !(c->p_mut >= 0.f && c->p_mut <= 1.f)) return ME_ERR_RANGE;
     if (c->pixel_id_base < 0 || N < 0 || (uint64_t)c->pixel_id_base + (uint64_t)N > 0x100000000ULL) return ME_ERR_RANGE;
     std::memset(&g, 0, sizeof(g));
@@ -97,6 +121,10 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
             g.log2ratio[j] = (float)std::log2((double)c->hi[j] / (double)c->lo[j]);
         }
     }
+    g.variant = c->variant;
+    g.n_samp = c->generations / 4 > 1 ? c->generations / 4 : 1;
+    for (int j = 0; j < ME_MAX_NPAR; ++j) sobol_directions16(j, g.sobol_v[j]);
+    if (c->variant == 1) return ME_OK;                        // the mutation-scale schedule is not used
     if (c->mut_scale_table != nullptr) {
         for (int t = 0; t <= c->generations; ++t) g.mut_scale[t] = c->mut_scale_table[t];
     } else {

@@ -51,6 +51,10 @@ struct GaDesc {
     float lo[ME_MAX_NPAR], span[ME_MAX_NPAR], log2ratio[ME_MAX_NPAR];
     int log_scale[ME_MAX_NPAR], periodic[ME_MAX_NPAR];
     float mut_scale[ME_MAX_GEN + 1];    // s_t, t = 0..generations
+    // variant 1 (the paper's binary-coded GA, readings V0-V5 of DESIGN.md)
+    int variant;                        // 0 real-coded operators, 1 binary-coded
+    int n_samp;                         // restart period max(1, G / 4)
+    uint32_t sobol_v[ME_MAX_NPAR][16];  // Sobol' direction numbers v_1..v_16 per dimension (point indices < 2^16)
 };
 
 // ------------------------------------------------------------------------------------------------------------
@@ -370,6 +374,97 @@ __device__ __forceinline__ uint32_t lane_of(const uint4& r, int k) {
 __device__ __forceinline__ float decode_gene(float g, const GaDesc& c, int j) {
     if (c.log_scale[j]) return c.lo[j] * exp2f(g * c.log2ratio[j]);
     return fmaf(c.span[j], g, c.lo[j]);
+}
+
+// Gene value in [0,1] from the stored gene: the real-coded variant stores it; the binary-coded variant stores the 16-bit
+// code k as an integer-valued float and decodes g = k / (2^16 - 1) (eq. 5) with one IEEE division.
+__device__ __forceinline__ float gene_value(float stored, const GaDesc& c) {
+    return c.variant ? __fdiv_rn(stored, 65535.0f) : stored;
+}
+
+// ---- variant 1: Sobol' points (Bratley & Fox 1988 as the paper uses them) -----------------------
+// Point n of dimension j in Gray-code order, top 16 bits, xor the per-pixel digital shift (reading V1).
+template <int M>
+__device__ __forceinline__ void sobol_genes(float* g, uint32_t pixel, uint32_t n, const GaDesc& c) {
+    const uint32_t gray = n ^ (n >> 1);
+    uint4 r = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+        if ((j & 3) == 0) r = philox4x32_10(pixel, 0u, 0xFFFFFFFFu, (uint32_t)(j >> 2), c.key0, c.key1);
+        uint32_t x = 0, q = gray;
+        while (q) {
+            const int b = __ffs(q) - 1;
+            x ^= c.sobol_v[j][b];
+            q &= q - 1;
+        }
+        g[j] = (float)(((x >> 16) ^ (lane_of(r, j & 3) >> 16)) & 0xFFFFu);
+    }
+}
+
+__device__ __forceinline__ int tournament(const uint4& r, const float* chi2, const GaDesc& c);
+
+// k-way tournament among the n_live best (order[rank] = member index); reading V2/V3.
+__device__ __forceinline__ int tournament_live(const uint4& r, const float* chi2, const uint16_t* order, int n_live,
+                                               const GaDesc& c) {
+    int best = order[below(r.x, n_live)];
+    float fb = chi2[best];
+    for (int m = 1; m < c.tournament_k; ++m) {
+        const int cand = order[below(lane_of(r, m), n_live)];
+        const float fc = chi2[cand];
+        if (fc < fb || (fc == fb && cand < best)) { best = cand; fb = fc; }
+    }
+    return best;
+}
+
+// Child i >= 1 of generation t, binary-coded (readings V2, V4, V5).  order == nullptr: every member is live.
+template <int M>
+__device__ __forceinline__ void make_child_binary(float* child, const float* genes, const float* chi2,
+                                                  const uint16_t* order, int n_live, uint32_t pixel, uint32_t t,
+                                                  uint32_t i, const GaDesc& c) {
+    if ((int)i >= n_live) {                                   // restart: the next points of the shifted Sobol' sequence
+        const int n_dead = c.pop - n_live;
+        sobol_genes<M>(child, pixel, (uint32_t)(c.pop + ((int)t / c.n_samp - 1) * n_dead + ((int)i - n_live) + 1), c);
+        return;
+    }
+    const uint32_t key = 2u * ((i + 1u) >> 1) - 1u;           // the pair (2q-1, 2q) shares its parents and its cut
+    int A, B;
+    if (order != nullptr) {
+        A = tournament_live(philox4x32_10(pixel, t, key, 0u, c.key0, c.key1), chi2, order, n_live, c);
+        B = tournament_live(philox4x32_10(pixel, t, key, 1u, c.key0, c.key1), chi2, order, n_live, c);
+    } else {
+        A = tournament(philox4x32_10(pixel, t, key, 0u, c.key0, c.key1), chi2, c);
+        B = tournament(philox4x32_10(pixel, t, key, 1u, c.key0, c.key1), chi2, c);
+    }
+    const uint4 rc = philox4x32_10(pixel, t, key, 2u, c.key0, c.key1);
+    const bool cross = u01(rc.x) < c.p_cross;
+    const int cut = 1 + below(rc.y, 16 * M - 1);
+    const int first = (i & 1u) ? A : B, second = (i & 1u) ? B : A;
+    uint4 rm = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+        const uint32_t k1 = (uint32_t)genes[first * M + j], k2 = (uint32_t)genes[second * M + j];
+        uint32_t k = k1;
+        if (cross) {
+            const int nhead = min(max(cut - 16 * j, 0), 16);  // bits taken from the first parent, MSB side
+            const uint32_t mask = (0xFFFFu << (16 - nhead)) & 0xFFFFu;
+            k = (k1 & mask) | (k2 & ~mask & 0xFFFFu);
+        }
+        if ((j & 1) == 0) rm = philox4x32_10(pixel, t, i, (uint32_t)(3 + j / 2), c.key0, c.key1);
+        const uint32_t xm = (j & 1) ? rm.z : rm.x, xd = (j & 1) ? rm.w : rm.y;
+        if (u01(xm) < c.p_mut) k ^= ((xd & 0xFFFFu) & (xd >> 16)) >> (xm & 15u);
+        child[j] = (float)k;
+    }
+}
+
+// Rank of member i by (chi2, index): the number of members that come before it.  O(pop) shared-memory reads.
+__device__ __forceinline__ int rank_of(const float* chi2, int pop, int i) {
+    const float fi = chi2[i];
+    int r = 0;
+    for (int k = 0; k < pop; ++k) {
+        const float fk = chi2[k];
+        r += (fk < fi || (fk == fi && k < i)) ? 1 : 0;
+    }
+    return r;
 }
 
 // generation 0, gene j: lane (j mod 4) of block floor(j / 4)

@@ -17,7 +17,7 @@ __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDe
                                          const float4* obs_s, const float2* nm_s) {
     float p[M];
 #pragma unroll
-    for (int j = 0; j < M; ++j) p[j] = decode_gene(g[j], gd, j);
+    for (int j = 0; j < M; ++j) p[j] = decode_gene(gene_value(g[j], gd), gd, j);
     Individual<NL> ind;
     setup_individual<NL, M>(ind, p, mu, sd);
     f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
@@ -63,6 +63,7 @@ __device__ __forceinline__ void stage_nm(float2* nm_s, const float* nm, int L, i
 // ------------------------------------------------------------------------------------------------------------
 // The fused GA inversion kernel.
 // Dynamic shared memory: obs_s [ceil(L/2)] 2 x float4 | nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] | scratch [64]
+//                        | order [pop] u16 (variant 1: members ranked by chi2 at restart generations)
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET, int M, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -77,6 +78,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
     float* chi2_s = genes_s + 2 * pop * M;
     if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, threadIdx.x, THREADS);     // once per CTA; synced below
     uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + 2 * pop);
+    uint16_t* order_s = reinterpret_cast<uint16_t*>(scratch + 64);
     const int tid = threadIdx.x;
     const float INF = __int_as_float(0x7f800000);
 
@@ -104,15 +106,25 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
             const float* gprev = genes_s + cur * pop * M;
             const float* fprev = chi2_s + cur * pop;
             float* gnext = genes_s + (cur ^ 1) * pop * M;
+            // variant 1, restart generation (reading V2): rank the previous generation; the worst half is dead
+            const bool restart = gd.variant != 0 && t > 0 && t < gd.generations && (t % gd.n_samp) == 0;
+            if (restart) {
+                if (alive) order_s[rank_of(fprev, pop, tid)] = (uint16_t)tid;
+                __syncthreads();
+            }
             if (alive) {
                 bool evaluate = true;
                 if (t == 0) {
-                    init_genes<M>(g, pixel, (uint32_t)tid, gd);                       // reading G2
+                    if (gd.variant) sobol_genes<M>(g, pixel, (uint32_t)tid + 1u, gd);  // reading V1
+                    else init_genes<M>(g, pixel, (uint32_t)tid, gd);                  // reading G2
                 } else if (tid == 0) {
 #pragma unroll
                     for (int j = 0; j < M; ++j) g[j] = gprev[ie * M + j];
                     f = fe;                                // carried, not re-evaluated (reading G3)
                     evaluate = false;
+                } else if (gd.variant) {
+                    make_child_binary<M>(g, gprev, fprev, restart ? order_s : nullptr, restart ? pop - pop / 2 : pop, pixel,
+                                         (uint32_t)t, (uint32_t)tid, gd);
                 } else {
                     make_child<M>(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
                 }
@@ -129,7 +141,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         block_argmin(f, tid, scratch, fe, ie);             // reading G5
         if (tid == ie) {
 #pragma unroll
-            for (int j = 0; j < M; ++j) out_params[n * M + j] = decode_gene(g[j], gd, j);
+            for (int j = 0; j < M; ++j) out_params[n * M + j] = decode_gene(gene_value(g[j], gd), gd, j);
             out_chi2[n] = f;
         }
     }
@@ -268,7 +280,8 @@ template <int NL, bool TRIPLET, int M, int THREADS, int MINB>
 static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask,
                                       const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
     auto k = ga_invert_kernel<NL, TRIPLET, M, THREADS, MINB>;
-    const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * M * 4 + (size_t)2 * gd.pop * 4 + 64 * 4;
+    const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * M * 4 + (size_t)2 * gd.pop * 4 + 64 * 4 +
+                        (size_t)2 * gd.pop + 16;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid_for_(N), THREADS, smem, st>>>(sd, gd, obs, mask, mu, N, out_params, out_chi2);

@@ -27,7 +27,9 @@ __global__ void ga_step_kernel(const __grid_constant__ GaDesc gd, const float* _
     float* genes_s = reinterpret_cast<float*>(smem4);
     float* chi2_s = genes_s + pop * M;
     uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + pop);
+    uint16_t* order_s = reinterpret_cast<uint16_t*>(scratch + 64);
     const float INF = __int_as_float(0x7f800000);
+    const bool restart = gd.variant != 0 && t < gd.generations && (t % gd.n_samp) == 0;
     for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
         __syncthreads();
         for (int k = tid; k < pop * M; k += blockDim.x) genes_s[k] = genes_in[n * pop * M + k];
@@ -40,11 +42,18 @@ __global__ void ga_step_kernel(const __grid_constant__ GaDesc gd, const float* _
         __syncthreads();
         float fe; int ie;
         block_argmin(f, tid, scratch, fe, ie);
+        if (restart) {
+            if (tid < pop) order_s[rank_of(chi2_s, pop, tid)] = (uint16_t)tid;
+            __syncthreads();
+        }
         if (tid < pop) {
             float g[M];
             if (tid == 0) {
 #pragma unroll
                 for (int j = 0; j < M; ++j) g[j] = genes_s[ie * M + j];
+            } else if (gd.variant) {
+                make_child_binary<M>(g, genes_s, chi2_s, restart ? order_s : nullptr, restart ? pop - pop / 2 : pop,
+                                     gd.pixel_base + (uint32_t)n, (uint32_t)t, (uint32_t)tid, gd);
             } else {
                 make_child<M>(g, genes_s, chi2_s, gd.pixel_base + (uint32_t)n, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
             }
@@ -61,7 +70,8 @@ __global__ void ga_init_kernel(const __grid_constant__ GaDesc gd, int64_t N, flo
     const int64_t n = k / gd.pop;
     const int i = (int)(k - n * gd.pop);
     float g[M];
-    init_genes<M>(g, gd.pixel_base + (uint32_t)n, (uint32_t)i, gd);
+    if (gd.variant) sobol_genes<M>(g, gd.pixel_base + (uint32_t)n, (uint32_t)i + 1u, gd);
+    else init_genes<M>(g, gd.pixel_base + (uint32_t)n, (uint32_t)i, gd);
 #pragma unroll
     for (int j = 0; j < M; ++j) genes_out[k * M + j] = g[j];
 }
@@ -132,7 +142,7 @@ cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* 
 cudaError_t launch_ga_step(const GaDesc& gd, int npar, const float* genes_in, const float* chi2_in, int64_t N, int t,
                            float* genes_out, cudaStream_t st) {
     const int threads = ((gd.pop + 31) / 32) * 32;
-    const size_t smem = (size_t)gd.pop * npar * 4 + (size_t)gd.pop * 4 + 64 * 4;
+    const size_t smem = (size_t)gd.pop * npar * 4 + (size_t)gd.pop * 4 + 64 * 4 + (size_t)2 * gd.pop + 16;
     if (npar == ME_MAX_NPAR) ga_step_kernel<ME_MAX_NPAR><<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
     else ga_step_kernel<ME_NPAR><<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
     return cudaGetLastError();
