@@ -94,6 +94,17 @@ def _variant(cfg):
     return int(cfg.get("variant", 0))
 
 
+def prologue(obs, cfg):
+    """obs[N,4,L] -> [N,6]: w_I, w_Q, w_U, w_V (eq. 20-23) and the inclination box, per cfg["prologue"] bits."""
+    obs = _f64(obs)
+    N, L = obs.shape[0], obs.shape[2]
+    w, sg = _f64(cfg["stokes_weight"]), _f64(cfg["sigma"])
+    out = np.empty((N, 6))
+    lib().orc_prologue(_p(obs, C.c_double), C.c_int64(N), C.c_int(L), _p(w, C.c_double), _p(sg, C.c_double),
+                       C.c_double(cfg["lo"][1]), C.c_double(cfg["hi"][1]), C.c_int(int(cfg.get("prologue", 0))), _p(out, C.c_double))
+    return out
+
+
 def sobol(n0, count, dims):
     out = np.zeros((count, dims), dtype=np.uint32)
     lib().orc_sobol(C.c_uint32(n0), C.c_int(count), C.c_int(dims), _p(out, C.c_uint32))
@@ -223,6 +234,6 @@ def ga_invert(obs, lam, lines, cfg, seed, mask=None, mu=None, pixel_base=0, thre
     lib().orc_ga_invert(_p(obs, C.c_double), _p(mask_a, C.c_ubyte), _p(mu_a, C.c_double), C.c_int64(N), C.c_uint64(pixel_base),
                         _p(lam, C.c_double), C.c_int(L), *lines.args(), *a,
                         _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(per, C.c_int),
-                        _p(w, C.c_double), _p(sg, C.c_double), C.c_int(npar), C.c_int(_variant(cfg)), _p(nm, C.c_double), C.c_uint64(seed), C.c_int(threads),
+                        _p(w, C.c_double), _p(sg, C.c_double), C.c_int(npar), C.c_int(_variant(cfg)), C.c_int(int(cfg.get("prologue", 0))), _p(nm, C.c_double), C.c_uint64(seed), C.c_int(threads),
                         _p(params, C.c_double), _p(chi2v, C.c_double), _p(genes, C.c_float), _p(trace, C.c_double))
     return {"params": params, "chi2": chi2v, "genes": genes, "trace": trace}

@@ -35,8 +35,8 @@ template <class F> void parallel_for(int64_t n, int threads, F f) {
 
 GaCfg make_cfg(int pop, int generations, int tournament_k, float p_cross, float p_mut, const float* mut_scale,
                const double* lo, const double* hi, const int* log_scale, const int* periodic,
-               const double* w, const double* sigma, uint64_t seed, int npar = NPAR, const double* nm_profile = nullptr, int variant = 0) {
-    GaCfg c; c.variant = variant; c.npar = npar; c.nm_profile = nm_profile; c.pop = pop; c.generations = generations; c.tournament_k = tournament_k;
+               const double* w, const double* sigma, uint64_t seed, int npar = NPAR, const double* nm_profile = nullptr, int variant = 0, int prologue = 0) {
+    GaCfg c; c.prologue = prologue; c.variant = variant; c.npar = npar; c.nm_profile = nm_profile; c.pop = pop; c.generations = generations; c.tournament_k = tournament_k;
     c.p_cross = p_cross; c.p_mut = p_mut; c.mut_scale.assign(mut_scale, mut_scale + generations + 1);
     for (int j = 0; j < npar; ++j) { c.lo[j] = lo[j]; c.hi[j] = hi[j]; c.log_scale[j] = log_scale[j]; c.periodic[j] = periodic[j]; }
     for (int s = 0; s < 4; ++s) { c.w[s] = w[s]; c.sigma[s] = sigma[s]; }
@@ -94,6 +94,15 @@ void orc_philox(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c
     uint32_t ctr[4] = { c0, c1, c2, c3 }, key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
     philox4x32_10(ctr, key, out);
 }
+// Per-pixel prologue: obs[N][4][L] -> out[N][6] (w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi).
+void orc_prologue(const double* obs, int64_t N, int L, const double* w, const double* sigma, double gamma_lo, double gamma_hi,
+                  int prologue, double* out) {
+    GaCfg c; c.prologue = prologue;
+    for (int s = 0; s < 4; ++s) { c.w[s] = w[s]; c.sigma[s] = sigma[s]; }
+    c.lo[P_GAMMA] = gamma_lo; c.hi[P_GAMMA] = gamma_hi;
+    for (int64_t n = 0; n < N; ++n) pixel_prologue(obs + n * 4 * L, L, c, out + n * 6);
+}
+
 // count Sobol' points starting at index n0, dims dimensions: out[count][dims] (32-bit fixed point).
 void orc_sobol(uint32_t n0, int count, int dims, uint32_t* out) {
     for (int i = 0; i < count; ++i)
@@ -148,10 +157,10 @@ void orc_ga_invert(const double* obs, const unsigned char* mask, const double* m
                    const double* shift, const double* weight, const int* kind, double lambda_ref,
                    int pop, int generations, int tournament_k, float p_cross, float p_mut, const float* mut_scale,
                    const double* lo, const double* hi, const int* log_scale, const int* periodic,
-                   const double* w, const double* sigma, int npar, int variant, const double* nm_profile, uint64_t seed, int threads,
+                   const double* w, const double* sigma, int npar, int variant, int prologue, const double* nm_profile, uint64_t seed, int threads,
                    double* out_params, double* out_chi2, float* out_genes, double* trace) {
     Lines ln = make_lines(n_lines, lambda0, strength, n_comp, shift, weight, kind, lambda_ref);
-    GaCfg c = make_cfg(pop, generations, tournament_k, p_cross, p_mut, mut_scale, lo, hi, log_scale, periodic, w, sigma, seed, npar, nm_profile, variant);
+    GaCfg c = make_cfg(pop, generations, tournament_k, p_cross, p_mut, mut_scale, lo, hi, log_scale, periodic, w, sigma, seed, npar, nm_profile, variant, prologue);
     parallel_for(N, threads, [&](int64_t n) {
         if (mask && !mask[n]) {
             for (int j = 0; j < npar; ++j) out_params[n * npar + j] = std::nan("");

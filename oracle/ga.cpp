@@ -183,8 +183,47 @@ static double fitness(const float* g, const double* obs, double mu, const double
     return x;
 }
 
-void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c,
+// W1 (eq. 20-23): w_I = 1 / (I_c - I_0), w_Q,U,V = 1 / max |Q,U,V|, with I_c the largest and I_0 the
+//    smallest observed intensity of the window (continuum and line core); each denominator is floored at the noise
+//    level sigma_s so that an empty Stokes parameter cannot blow the weight up; as for the fixed weights (reading F11)
+//    the weight enters eq. 16 as (w_s / sigma_s)^2.
+// P1: the inclination box is cut to one polarity, "in agreement with the order of the blue- and
+//    red-lobes of the observed Stokes V": if the maximum of V lies at a shorter wavelength than its minimum (first
+//    occurrences) the blue lobe is positive, which is gamma < 90 deg (reading F4): box [lo, min(hi, 90)]; else
+//    [max(lo, 90), hi].
+void pixel_prologue(const double* obs, int L, const GaCfg& c, double out[6]) {
+    for (int s = 0; s < 4; ++s) out[s] = c.w[s];
+    out[4] = c.lo[P_GAMMA]; out[5] = c.hi[P_GAMMA];
+    if (c.prologue & 1) {
+        double imax = obs[0], imin = obs[0];
+        for (int j = 1; j < L; ++j) { imax = std::fmax(imax, obs[j]); imin = std::fmin(imin, obs[j]); }
+        out[0] = 1.0 / std::fmax(imax - imin, c.sigma[0]);
+        for (int s = 1; s < 4; ++s) {
+            double m = 0.0;
+            for (int j = 0; j < L; ++j) m = std::fmax(m, std::fabs(obs[s * L + j]));
+            out[s] = 1.0 / std::fmax(m, c.sigma[s]);
+        }
+    }
+    if (c.prologue & 2) {
+        int jmax = 0, jmin = 0;
+        for (int j = 1; j < L; ++j) {
+            if (obs[3 * L + j] > obs[3 * L + jmax]) jmax = j;
+            if (obs[3 * L + j] < obs[3 * L + jmin]) jmin = j;
+        }
+        if (jmax < jmin) out[5] = std::fmin(c.hi[P_GAMMA], 90.0);
+        else out[4] = std::fmax(c.lo[P_GAMMA], 90.0);
+    }
+}
+
+void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c0,
                      uint64_t pixel, double* best_params, double* best_chi2, float* best_genes, double* trace) {
+    GaCfg c = c0;                                                  // per-pixel weights and inclination box
+    if (c0.prologue) {
+        double pr[6];
+        pixel_prologue(obs, L, c0, pr);
+        for (int s = 0; s < 4; ++s) c.w[s] = pr[s];
+        c.lo[P_GAMMA] = pr[4]; c.hi[P_GAMMA] = pr[5];
+    }
     const int M = c.npar;
     std::vector<float> genes(c.pop * M), next(c.pop * M);
     std::vector<double> f(c.pop), fnext(c.pop), model(4 * L);

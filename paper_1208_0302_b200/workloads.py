@@ -46,13 +46,13 @@ def mutation_schedule(generations, s0=0.5, s_end=0.0025):
 
 
 def ga_config(pop, generations, sigma=1e-3, b_lo=10.0, b_hi=3000.0, tournament_k=3, p_cross=0.8, p_mut=None,
-              s0=0.5, s_end=0.0025, stokes_weight=(1.0, 4.0, 4.0, 2.0), npar=NPAR, variant=0):
+              s0=0.5, s_end=0.0025, stokes_weight=(1.0, 4.0, 4.0, 2.0), npar=NPAR, variant=0, prologue=0):
     lo, hi, log_scale, periodic = prior_box(b_lo, b_hi, npar)
     return dict(pop=int(pop), generations=int(generations), tournament_k=int(tournament_k),
                 p_cross=float(np.float32(p_cross)), p_mut=float(np.float32(2.0 / npar if p_mut is None else p_mut)),
                 mut_scale=mutation_schedule(generations, s0, s_end), lo=lo, hi=hi, log_scale=log_scale, periodic=periodic,
                 stokes_weight=np.asarray(stokes_weight, dtype=np.float64), sigma=np.full(4, float(sigma)),
-                variant=int(variant))
+                variant=int(variant), prologue=int(prologue))
 
 
 def draw_truth(n, seed=SEED_TRUTH, b_lo=10.0, b_hi=3000.0, stream=0, npar=NPAR):
