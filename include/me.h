@@ -107,7 +107,13 @@ typedef struct {
                                     (PAPER.md:103-105), Sobol' initial population and re-seeding of the worst half
                                     every max(1, G/4) generations. mut_scale* are ignored.
                                     In the test hooks a gene then holds its code k in [0, 65535] as a float. */
-    int reserved;             /* must be 0 */
+    int prologue;             /* per-pixel prologue of the paper, bit flags (readings W1, P1):
+                                 1: inverse-max weights, eq. 20-23: w_I = 1/(I_c - I_0), w_Q,U,V =
+                                    1/max|Q,U,V| from the observed profile (denominators floored at sigma_s) replace
+                                    stokes_weight;
+                                 2: the inclination box [lo[1], hi[1]] is cut to the polarity given by the order of the
+                                    Stokes-V lobes: positive lobe on the blue side => gamma <= 90 deg.
+                                 ga_fitness ignores these flags (fixed weights, configured box). */
 } ga_cfg;
 
 /* GA inversion of N pixels.
@@ -128,6 +134,9 @@ int ga_step(const float* genes_in /*[N,pop,n_params]*/, const float* chi2_in /*[
 int ga_fitness(const float* genes /*[N,pop,n_params]*/, const float* obs /*[N,4,L]*/, int64_t N, const float* sigma /*host[4]*/,
                const double* lambda_grid_A, int L, const me_line_data* line_data, const ga_cfg* cfg,
                float* chi2_out /*[N,pop]*/, void* stream);
+/* The per-pixel prologue alone: out device [N,6] f32 = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them. */
+int ga_prologue(const float* obs /*[N,4,L]*/, int64_t N, int L, const float* sigma /*host[4]*/, const ga_cfg* cfg,
+                float* out, void* stream);
 /* Generation-0 population (reading G2): genes_out device [N,pop,n_params]. */
 int ga_init(int64_t N, const ga_cfg* cfg, int n_params, uint64_t seed, float* genes_out, void* stream);
 /* One Philox4x32-10 block computed ON THE DEVICE; out is a HOST pointer; synchronises. */

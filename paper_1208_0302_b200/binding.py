@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libme_b200.so")
 _lib = None
 
-EXPORTS = ["me_synth", "ga_invert", "ga_step", "ga_fitness", "ga_init", "me_philox", "me_philox_many", "me_faddeeva",
+EXPORTS = ["me_synth", "ga_invert", "ga_step", "ga_fitness", "ga_init", "ga_prologue", "me_philox", "me_philox_many", "me_faddeeva",
            "me_zeeman_pattern", "me_peak_probe", "me_strerror", "me_last_cuda_error", "me_version"]
 
 
@@ -46,7 +46,7 @@ class _GaCfg(C.Structure):
                 ("lo", C.c_float * MAX_NPAR), ("hi", C.c_float * MAX_NPAR),
                 ("log_scale", C.c_uint8 * MAX_NPAR), ("periodic", C.c_uint8 * MAX_NPAR),
                 ("stokes_weight", C.c_float * 4), ("mu", C.c_void_p), ("pixel_id_base", C.c_int64),
-                ("variant", C.c_int), ("reserved", C.c_int)]
+                ("variant", C.c_int), ("prologue", C.c_int)]
 
 
 def lib():
@@ -151,7 +151,7 @@ def make_ga_cfg(cfg, mu=None, pixel_id_base=0):
     c.mu = _dev(mu, torch.float32, "mu").value if mu is not None else None
     c.pixel_id_base = int(pixel_id_base)
     c.variant = int(cfg.get("variant", 0))
-    c.reserved = 0
+    c.prologue = int(cfg.get("prologue", 0))
     return c, (ms, mu)
 
 
@@ -265,3 +265,15 @@ def me_peak_probe(kind, iters, blocks, scratch):
     _check(lib().me_peak_probe(C.c_int(kind), C.c_int(iters), C.c_int(blocks), _dev(scratch, torch.float32, "out"), _stream()),
            "me_peak_probe")
     return blocks * 256 * iters * 32
+
+
+def ga_prologue(obs, cfg):
+    """obs: CUDA f32 [N,4,L]. Returns [N,6]: w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them (cfg["prologue"])."""
+    import torch
+    N, L = obs.shape[0], obs.shape[2]
+    c, keep = make_ga_cfg(cfg)
+    sig = np.ascontiguousarray(cfg["sigma"], dtype=np.float32)
+    out = torch.empty((N, 6), dtype=torch.float32, device=obs.device)
+    _check(lib().ga_prologue(_dev(obs, torch.float32, "obs"), C.c_int64(N), C.c_int(L), sig.ctypes.data_as(C.POINTER(C.c_float)),
+                             C.byref(c), _dev(out, torch.float32, "out"), _stream()), "ga_prologue")
+    return out

@@ -95,7 +95,8 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
     if (c->tournament_k < 1 || c->tournament_k > 4) return ME_ERR_RANGE;
     if (c->elite != 1) return ME_ERR_UNSUPPORTED;
     if (c->variant != 0 && c->variant != 1) return ME_ERR_RANGE;
-    if (c->reserved != 0) return ME_ERR_RANGE;
+    if (c->prologue < 0 || c->prologue > 3) return ME_ERR_RANGE;
+    if ((c->prologue & 2) && c->log_scale[1]) return ME_ERR_UNSUPPORTED;      // the polarity box is linear in gamma
     if (!(c->p_cross >= 0.f && c->p_cross <= 1.f) || !(c->p_mut >= 0.f && c->p_mut <= 1.f)) return ME_ERR_RANGE;
     if (c->pixel_id_base < 0 || N < 0 || (uint64_t)c->pixel_id_base + (uint64_t)N > 0x100000000ULL) return ME_ERR_RANGE;
     std::memset(&g, 0, sizeof(g));
@@ -109,6 +110,8 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
         if (!(sg > 0.0) || !(c->stokes_weight[s] >= 0.f)) return ME_ERR_RANGE;
         double w = (double)c->stokes_weight[s] / sg;
         g.w2[s] = (float)(w * w);
+        g.w_cfg[s] = c->stokes_weight[s];
+        g.sigma[s] = (float)sg;
     }
     for (int j = 0; j < npar; ++j) {
         if (!(c->lo[j] <= c->hi[j])) return ME_ERR_RANGE;
@@ -121,6 +124,7 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
             g.log2ratio[j] = (float)std::log2((double)c->hi[j] / (double)c->lo[j]);
         }
     }
+    g.prologue = c->prologue;
     g.variant = c->variant;
     g.n_samp = c->generations / 4 > 1 ? c->generations / 4 : 1;
     for (int j = 0; j < ME_MAX_NPAR; ++j) sobol_directions16(j, g.sobol_v[j]);
@@ -214,6 +218,17 @@ int ga_step(const float* genes_in, const float* chi2_in, int64_t N, int generati
     if (N == 0) return ME_OK;
     if (genes_in == nullptr || chi2_in == nullptr || genes_out == nullptr) return ME_ERR_NULL;
     cudaError_t e = me::launch_ga_step(gd, n_params, genes_in, chi2_in, N, generation, genes_out, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int ga_prologue(const float* obs, int64_t N, int L, const float* sigma, const ga_cfg* cfg, float* out, void* stream) {
+    if (L < 2 || L > ME_MAX_L) return ME_ERR_SHAPE;
+    me::GaDesc gd;
+    int rc = build_ga_desc(cfg, ME_NPAR, sigma, L, 0, N, true, gd);
+    if (rc != ME_OK) return rc;
+    if (N == 0) return ME_OK;
+    if (obs == nullptr || out == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_ga_prologue(gd, obs, N, L, out, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 

@@ -51,6 +51,9 @@ struct GaDesc {
     float lo[ME_MAX_NPAR], span[ME_MAX_NPAR], log2ratio[ME_MAX_NPAR];
     int log_scale[ME_MAX_NPAR], periodic[ME_MAX_NPAR];
     float mut_scale[ME_MAX_GEN + 1];    // s_t, t = 0..generations
+    // per-pixel prologue (readings W1, P1): bit 0 inverse-max weights, bit 1 polarity restriction
+    int prologue;
+    float w_cfg[4], sigma[4];           // configured w_s and sigma_s (w2 above is (w_s / sigma_s)^2)
     // variant 1 (the paper's binary-coded GA, readings V0-V5 of DESIGN.md)
     int variant;                        // 0 real-coded operators, 1 binary-coded
     int n_samp;                         // restart period max(1, G / 4)
@@ -512,6 +515,64 @@ __device__ __forceinline__ void make_child(float* child, const float* genes, con
         if (c.periodic[j]) g = __fsub_rn(g, floorf(g));
         else g = fminf(fmaxf(g, 0.0f), 1.0f);
         child[j] = g;
+    }
+}
+
+// Stage obs[n] ([4][L] in HBM, rows contiguous => coalesced) into shared memory, pair-interleaved:
+// element (s, j) -> word 8 (j/2) + 2 s + (j & 1).  Shared size: 8 * ceil(L/2) floats.
+__device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int L, int tid, int nthreads) {
+    for (int k = tid; k < 4 * L; k += nthreads) {
+        const int s = k / L, j = k - s * L;
+        obs_s[8 * (j >> 1) + 2 * s + (j & 1)] = __ldg(obs_n + k);
+    }
+}
+
+// Per-pixel prologue (readings W1, P1; eq. 20-23, polarity PAPER.md:278), run by ONE warp on the staged
+// observation (pair-interleaved layout of stage_obs).  pix[0..3] = (w_s / sigma_s)^2, pix[4] = gamma_lo, pix[5] = gamma
+// span, pix[6] = gamma_hi; without flags these are the configured values.
+#define ME_PIX_WORDS 8
+__device__ __forceinline__ void pixel_prologue(const float* obs_s, int L, const GaDesc& gd, float* pix, bool writer) {
+    const int lane = threadIdx.x & 31;
+    const float INF = __int_as_float(0x7f800000);
+    float imax = -INF, imin = INF, mq = 0.f, mu_ = 0.f, mv = 0.f, vmax = -INF, vmin = INF;
+    int jmax = 0x7fffffff, jmin = 0x7fffffff;
+#pragma unroll 1
+    for (int j = lane; j < L; j += 32) {                        // ascending j per lane: strict compare keeps the first
+        const float* o = obs_s + 8 * (j >> 1) + (j & 1);
+        const float I = o[0], Q = o[2], U = o[4], V = o[6];
+        imax = fmaxf(imax, I); imin = fminf(imin, I);
+        mq = fmaxf(mq, fabsf(Q)); mu_ = fmaxf(mu_, fabsf(U)); mv = fmaxf(mv, fabsf(V));
+        if (V > vmax) { vmax = V; jmax = j; }
+        if (V < vmin) { vmin = V; jmin = j; }
+    }
+#pragma unroll 1
+    for (int s = 16; s > 0; s >>= 1) {
+        imax = fmaxf(imax, __shfl_xor_sync(0xffffffffu, imax, s)); imin = fminf(imin, __shfl_xor_sync(0xffffffffu, imin, s));
+        mq = fmaxf(mq, __shfl_xor_sync(0xffffffffu, mq, s)); mu_ = fmaxf(mu_, __shfl_xor_sync(0xffffffffu, mu_, s));
+        mv = fmaxf(mv, __shfl_xor_sync(0xffffffffu, mv, s));
+        const float ov = __shfl_xor_sync(0xffffffffu, vmax, s); const int oj = __shfl_xor_sync(0xffffffffu, jmax, s);
+        if (ov > vmax || (ov == vmax && oj < jmax)) { vmax = ov; jmax = oj; }
+        const float pv = __shfl_xor_sync(0xffffffffu, vmin, s); const int pj = __shfl_xor_sync(0xffffffffu, jmin, s);
+        if (pv < vmin || (pv == vmin && pj < jmin)) { vmin = pv; jmin = pj; }
+    }
+    if (writer) {
+        float glo = gd.lo[1], ghi = __fadd_rn(gd.lo[1], gd.span[1]);
+        if (gd.prologue & 1) {
+            const float den[4] = {fmaxf(imax - imin, gd.sigma[0]), fmaxf(mq, gd.sigma[1]), fmaxf(mu_, gd.sigma[2]), fmaxf(mv, gd.sigma[3])};
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const float w = __fdiv_rn(__fdiv_rn(1.0f, den[s]), gd.sigma[s]);
+                pix[s] = w * w;
+            }
+        } else {
+#pragma unroll
+            for (int s = 0; s < 4; ++s) pix[s] = gd.w2[s];
+        }
+        if (gd.prologue & 2) {
+            if (jmax < jmin) ghi = fminf(ghi, 90.0f);
+            else glo = fmaxf(glo, 90.0f);
+        }
+        pix[4] = glo; pix[5] = (gd.prologue & 2) ? ghi - glo : gd.span[1]; pix[6] = ghi;
     }
 }
 

@@ -14,10 +14,11 @@ namespace me {
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET, int M>
 __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
-                                         const float4* obs_s, const float2* nm_s) {
+                                         const float4* obs_s, const float2* nm_s, const float* pix) {
     float p[M];
 #pragma unroll
     for (int j = 0; j < M; ++j) p[j] = decode_gene(gene_value(g[j], gd), gd, j);
+    if (!gd.log_scale[1]) p[1] = fmaf(pix[5], gene_value(g[1], gd), pix[4]);   // inclination: per-pixel box (reading P1)
     Individual<NL> ind;
     setup_individual<NL, M>(ind, p, mu, sd);
     f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
@@ -38,18 +39,10 @@ __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDe
         aI.x = fmaf(dI, dI, aI.x); aQ.x = fmaf(dQ, dQ, aQ.x); aU.x = fmaf(dU, dU, aU.x); aV.x = fmaf(dV, dV, aV.x);
     }
     const float sI = aI.x + aI.y, sQ = aQ.x + aQ.y, sU = aU.x + aU.y, sV = aV.x + aV.y;
-    float chi2 = gd.inv_nu * fmaf(gd.w2[0], sI, fmaf(gd.w2[1], sQ, fmaf(gd.w2[2], sU, gd.w2[3] * sV)));
+    const volatile float* pw = pix;      // per-pixel (w_s/sigma_s)^2, read HERE (volatile: not hoisted above the loop, where it would cost 4 registers)
+    float chi2 = gd.inv_nu * fmaf(pw[0], sI, fmaf(pw[1], sQ, fmaf(pw[2], sU, pw[3] * sV)));
     if (!(chi2 < __int_as_float(0x7f800000))) chi2 = __int_as_float(0x7f800000);   // NaN / Inf -> +Inf (reading G4)
     return chi2;
-}
-
-// Stage obs[n] ([4][L] in HBM, rows contiguous => coalesced) into shared memory, pair-interleaved:
-// element (s, j) -> word 8 (j/2) + 2 s + (j & 1).  Shared size: 8 * ceil(L/2) floats.
-__device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int L, int tid, int nthreads) {
-    for (int k = tid; k < 4 * L; k += nthreads) {
-        const int s = k / L, j = k - s * L;
-        obs_s[8 * (j >> 1) + 2 * s + (j & 1)] = __ldg(obs_n + k);
-    }
 }
 
 // Stage I_fixed[L] pair-wise: nm_s[jp] = (F[2jp], F[2jp+1]); the odd tail duplicates its single value.
@@ -62,8 +55,8 @@ __device__ __forceinline__ void stage_nm(float2* nm_s, const float* nm, int L, i
 
 // ------------------------------------------------------------------------------------------------------------
 // The fused GA inversion kernel.
-// Dynamic shared memory: obs_s [ceil(L/2)] 2 x float4 | nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] | scratch [64]
-//                        | order [pop] u16 (variant 1: members ranked by chi2 at restart generations)
+// Dynamic shared memory: scratch [64] | pix [8] (per-pixel weights and inclination box) | obs_s [ceil(L/2)] 2 x float4 |
+//                        nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] | order [pop] u16 (variant 1: ranks at restarts)
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET, int M, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -72,13 +65,15 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
                  int64_t N, float* __restrict__ out_params, float* __restrict__ out_chi2) {
     extern __shared__ float4 smem4[];
     const int L = sd.L, pop = gd.pop;
-    float* obs_s = reinterpret_cast<float*>(smem4);
+    // fixed offsets first (compile-time shared addresses, no pointer registers): scratch [64] | pix [8] | obs_s ...
+    uint32_t* scratch = reinterpret_cast<uint32_t*>(smem4);
+    float* pix_s = reinterpret_cast<float*>(scratch + 64);
+    float* obs_s = pix_s + ME_PIX_WORDS;
     float2* nm_s = reinterpret_cast<float2*>(obs_s + 8 * ((L + 1) >> 1));
     float* genes_s = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));
     float* chi2_s = genes_s + 2 * pop * M;
+    uint16_t* order_s = reinterpret_cast<uint16_t*>(chi2_s + 2 * pop);
     if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, threadIdx.x, THREADS);     // once per CTA; synced below
-    uint32_t* scratch = reinterpret_cast<uint32_t*>(chi2_s + 2 * pop);
-    uint16_t* order_s = reinterpret_cast<uint16_t*>(scratch + 64);
     const int tid = threadIdx.x;
     const float INF = __int_as_float(0x7f800000);
 
@@ -93,6 +88,8 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         const float mu = mu_arr != nullptr ? __ldg(mu_arr + n) : 1.0f;
         __syncthreads();                                   // previous pixel's shared memory is no longer read
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
+        __syncthreads();
+        pixel_prologue(obs_s, L, gd, pix_s, tid == 0);      // every warp reduces, thread 0 writes; visible after the next barrier
 
         // generations 0..G with ONE fitness call site (keeps the loop body inside the instruction cache)
         float g[M];
@@ -128,7 +125,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
                 } else {
                     make_child<M>(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
                 }
-                if (evaluate) f = fitness<NL, TRIPLET, M>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s);
+                if (evaluate) f = fitness<NL, TRIPLET, M>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s);
 #pragma unroll
                 for (int j = 0; j < M; ++j) gnext[tid * M + j] = g[j];
                 chi2_s[(cur ^ 1) * pop + tid] = f;
@@ -142,6 +139,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         if (tid == ie) {
 #pragma unroll
             for (int j = 0; j < M; ++j) out_params[n * M + j] = decode_gene(gene_value(g[j], gd), gd, j);
+            if (!gd.log_scale[1]) out_params[n * M + 1] = fmaf(pix_s[5], gene_value(g[1], gd), pix_s[4]);
             out_chi2[n] = f;
         }
     }
@@ -257,6 +255,9 @@ ga_fitness_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ 
     const int L = sd.L, pop = gd.pop, tid = threadIdx.x;
     float2* nm_s = reinterpret_cast<float2*>(obs_s + 8 * ((L + 1) >> 1));
     if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, tid, 128);
+    float* pix_s = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));               // fixed weights, configured box
+    if (tid < 4) pix_s[tid] = gd.w2[tid];
+    if (tid == 4) { pix_s[4] = gd.lo[1]; pix_s[5] = gd.span[1]; }
     for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
         __syncthreads();
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, 128);
@@ -266,7 +267,7 @@ ga_fitness_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ 
             float g[M];
 #pragma unroll
             for (int j = 0; j < M; ++j) g[j] = genes[(n * pop + i) * M + j];
-            chi2_out[n * pop + i] = fitness<NL, TRIPLET, M>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s);
+            chi2_out[n * pop + i] = fitness<NL, TRIPLET, M>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s);
         }
     }
 }
@@ -281,7 +282,7 @@ static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, con
                                       const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
     auto k = ga_invert_kernel<NL, TRIPLET, M, THREADS, MINB>;
     const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * M * 4 + (size_t)2 * gd.pop * 4 + 64 * 4 +
-                        (size_t)2 * gd.pop + 16;
+                        (size_t)2 * gd.pop + 16 + ME_PIX_WORDS * 4;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid_for_(N), THREADS, smem, st>>>(sd, gd, obs, mask, mu, N, out_params, out_chi2);
@@ -310,7 +311,7 @@ cudaError_t ME_INST_NAME(launch_ga_invert)(const SynthDesc& sd, const GaDesc& gd
 
 cudaError_t ME_INST_NAME(launch_ga_fitness)(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs,
                                             const float* mu, int64_t N, float* chi2_out, cudaStream_t st) {
-    const size_t smem = (size_t)40 * ((sd.L + 1) / 2);
+    const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + ME_PIX_WORDS * 4;
     ga_fitness_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid_for_(N), 128, smem, st>>>(sd, gd, genes, obs, mu, N, chi2_out);
     return cudaGetLastError();
 }

@@ -76,6 +76,23 @@ __global__ void ga_init_kernel(const __grid_constant__ GaDesc gd, int64_t N, flo
     for (int j = 0; j < M; ++j) genes_out[k * M + j] = g[j];
 }
 
+// The per-pixel prologue alone (one warp per pixel): out[n][6] = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi.
+__global__ void ga_prologue_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ obs, int64_t N, int L,
+                                   float* __restrict__ out) {
+    extern __shared__ float4 smem4[];
+    float* obs_s = reinterpret_cast<float*>(smem4);
+    float* pix_s = obs_s + 8 * ((L + 1) >> 1);
+    for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
+        __syncwarp();
+        stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, threadIdx.x, 32);
+        __syncwarp();
+        pixel_prologue(obs_s, L, gd, pix_s, threadIdx.x == 0);
+        __syncwarp();
+        if (threadIdx.x < 4) out[n * 6 + threadIdx.x] = sqrtf(pix_s[threadIdx.x]) * gd.sigma[threadIdx.x];   // back to w_s
+        if (threadIdx.x == 4) { out[n * 6 + 4] = pix_s[4]; out[n * 6 + 5] = pix_s[6]; }
+    }
+}
+
 __global__ void philox_kernel(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3,
                               int64_t n, uint4* __restrict__ out) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -152,6 +169,12 @@ cudaError_t launch_ga_init(const GaDesc& gd, int npar, int64_t N, float* genes_o
     const int64_t total = N * gd.pop;
     if (npar == ME_MAX_NPAR) ga_init_kernel<ME_MAX_NPAR><<<grid_for((total + 255) / 256), 256, 0, st>>>(gd, N, genes_out);
     else ga_init_kernel<ME_NPAR><<<grid_for((total + 255) / 256), 256, 0, st>>>(gd, N, genes_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ga_prologue(const GaDesc& gd, const float* obs, int64_t N, int L, float* out, cudaStream_t st) {
+    const size_t smem = (size_t)32 * ((L + 1) / 2) + ME_PIX_WORDS * 4;
+    ga_prologue_kernel<<<grid_for(N), 32, smem, st>>>(gd, obs, N, L, out);
     return cudaGetLastError();
 }
 
