@@ -105,6 +105,41 @@ def prologue(obs, cfg):
     return out
 
 
+def uncertainty(obs, params, lam, lines, cfg, mu=None, nm_profile=None, threads=1):
+    """eq. 26 / reading U1: obs[N,4,L], params[N,M] (the optimum) -> (sigma[N,M], chi2[N])."""
+    obs, lam, params = _f64(obs), _f64(lam), _f64(params)
+    N, L, npar = obs.shape[0], lam.size, _npar(cfg)
+    assert params.shape == (N, npar)
+    mu_a = _f64(mu) if mu is not None else None
+    nm = _nm(nm_profile, npar, L)
+    lo, hi, lg = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"])
+    w, sg = _f64(cfg["stokes_weight"]), _f64(cfg["sigma"])
+    sig, chi = np.empty((N, npar)), np.empty(N)
+    lib().orc_uncertainty(_p(obs, C.c_double), _p(mu_a, C.c_double), C.c_int64(N), _p(lam, C.c_double), C.c_int(L),
+                          *lines.args(), _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(w, C.c_double),
+                          _p(sg, C.c_double), C.c_int(npar), C.c_int(int(cfg.get("prologue", 0))), _p(nm, C.c_double),
+                          _p(params, C.c_double), C.c_int(threads), _p(sig, C.c_double), _p(chi, C.c_double))
+    return sig, chi
+
+
+def uncertainty_n_eval(M):
+    return int(lib().orc_uncertainty_n_eval(C.c_int(M)))
+
+
+def uncertainty_offsets(M, e, h):
+    du = np.zeros(M)
+    lib().orc_uncertainty_offsets(C.c_int(M), C.c_int(e), C.c_double(h), _p(du, C.c_double))
+    return du
+
+
+def uncertainty_from_chi2(chi2v, M, h, active=None):
+    chi2v = _f64(chi2v)
+    act = _i32(np.ones(M) if active is None else active)
+    out = np.empty(M)
+    lib().orc_uncertainty_from_chi2(_p(chi2v, C.c_double), C.c_int(M), C.c_double(h), _p(act, C.c_int), _p(out, C.c_double))
+    return out
+
+
 def sobol(n0, count, dims):
     out = np.zeros((count, dims), dtype=np.uint32)
     lib().orc_sobol(C.c_uint32(n0), C.c_int(count), C.c_int(dims), _p(out, C.c_uint32))

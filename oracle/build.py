@@ -7,7 +7,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["faddeeva.cpp", "zeeman.cpp", "synth.cpp", "philox.cpp", "sobol.cpp", "ga.cpp", "capi.cpp"]
+SOURCES = ["faddeeva.cpp", "zeeman.cpp", "synth.cpp", "philox.cpp", "sobol.cpp", "ga.cpp", "uncertainty.cpp", "capi.cpp"]
 LIB = os.path.join(HERE, "liboracle.so")
 
 

@@ -18,6 +18,7 @@
 //   philox4x32_10  pinned  (published known-answer vectors of Salmon et al. 2011)
 //   synth_n (11 parameters, reading F13) pinned (alpha=1,s=0 -> synth; alpha=0 -> B=0 closed form; s=1 -> I_fixed;
 //                  Q,U,V scale with (1-s) alpha; bilinearity in alpha and s)
+//   uncertainty    pinned  (exact Hessian of quadratic / quartic test functions, closed-form inverse; noise scaling)
 //   ga             operators pinned by brute-force re-derivation in Python on tiny inputs and by
 //                  invariants; absolute recovery accuracy: PARITY UNPINNED (the paper prints no
 //                  reproducible recovery numbers, Table 4 PAPER.md:340-345 is for SOLIS data).
@@ -106,5 +107,12 @@ void ga_init(uint64_t pixel, const GaCfg& c, float* genes);
 // if trace != nullptr it receives best chi2 per generation (generations+1 values).
 void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c,
                      uint64_t pixel, double* best_params, double* best_chi2, float* best_genes, double* trace);
+
+// ---- Uncertainties (eq. 25-26; reading U1 of DESIGN.md) ----
+int uncertainty_n_eval(int M);
+void uncertainty_offsets(int M, int e, double h, std::vector<double>& du);
+void uncertainty_from_chi2(const double* chi2v, int M, double h, const int* active, double* sigma_u);
+void uncertainty_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c,
+                       const double* params, double* sigma_p, double* chi2_opt);
 
 }  // namespace orc
