@@ -126,6 +126,17 @@ int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sig
               const double* lambda_grid_A, int L, const me_line_data* line_data, const ga_cfg* cfg, uint64_t seed,
               float* out_params, float* out_chi2, void* stream);
 
+/* Parameter uncertainties at the optimum (eq. 26; reading U1): the Hessian H of chi2 on the
+ * box coordinates (central second differences at h = 2^-7 and h/2, one Richardson/Neville level; 1 + 2(2M + 2M(M-1))
+ * syntheses per pixel through the same fused fitness as ga_invert), sigma_i^2 = [H^-1]_ii chi2(p_opt)/M, scaled to
+ * parameter units. Genes with lo == hi are left out (sigma = 0). A singular or indefinite Hessian gives NaN.
+ *   params     device [N, n_params] f32: the optimum (ga_invert's out_params)
+ *   out_sigma  device [N, n_params] f32        out_chi2  device [N] f32 or NULL: chi2 at params
+ * mask, sigma, cfg (boxes, weights, prologue flags, mu) as for ga_invert; the GA fields of cfg are ignored. */
+int ga_uncertainty(const float* obs, int64_t N, const uint8_t* mask, const float* sigma, const double* lambda_grid_A, int L,
+                   const me_line_data* line_data, const ga_cfg* cfg, const float* params, float* out_sigma, float* out_chi2,
+                   void* stream);
+
 /* Test hooks (not timed). */
 /* One generation t >= 1 of selection/crossover/mutation/elitism from given genes and given fitness. */
 int ga_step(const float* genes_in /*[N,pop,n_params]*/, const float* chi2_in /*[N,pop]*/, int64_t N, int generation,

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libme_b200.so")
 _lib = None
 
-EXPORTS = ["me_synth", "ga_invert", "ga_step", "ga_fitness", "ga_init", "ga_prologue", "me_philox", "me_philox_many", "me_faddeeva",
+EXPORTS = ["me_synth", "ga_invert", "ga_uncertainty", "ga_step", "ga_fitness", "ga_init", "ga_prologue", "me_philox", "me_philox_many", "me_faddeeva",
            "me_zeeman_pattern", "me_peak_probe", "me_strerror", "me_last_cuda_error", "me_version"]
 
 
@@ -277,3 +277,20 @@ def ga_prologue(obs, cfg):
     _check(lib().ga_prologue(_dev(obs, torch.float32, "obs"), C.c_int64(N), C.c_int(L), sig.ctypes.data_as(C.POINTER(C.c_float)),
                              C.byref(c), _dev(out, torch.float32, "out"), _stream()), "ga_prologue")
     return out
+
+
+def ga_uncertainty(obs, params, lam, line_data, cfg, mask=None, mu=None):
+    """obs: CUDA f32 [N,4,L]; params: CUDA f32 [N,M] (the optimum). Returns (sigma [N,M], chi2 [N]) per eq. 26."""
+    import torch
+    N = obs.shape[0]
+    lam, lam_p, L = _grid(lam)
+    assert tuple(params.shape) == (N, line_data.n_params) and len(cfg["lo"]) == line_data.n_params
+    c, keep = make_ga_cfg(cfg, mu)
+    sig = np.ascontiguousarray(cfg["sigma"], dtype=np.float32)
+    out_s = torch.empty((N, line_data.n_params), dtype=torch.float32, device=obs.device)
+    out_c = torch.empty((N,), dtype=torch.float32, device=obs.device)
+    _check(lib().ga_uncertainty(_dev(obs, torch.float32, "obs"), C.c_int64(N), _dev(mask, torch.uint8, "mask"),
+                                sig.ctypes.data_as(C.POINTER(C.c_float)), lam_p, L, C.byref(line_data.c), C.byref(c),
+                                _dev(params, torch.float32, "params"), _dev(out_s, torch.float32, "out_sigma"),
+                                _dev(out_c, torch.float32, "out_chi2"), _stream()), "ga_uncertainty")
+    return out_s, out_c

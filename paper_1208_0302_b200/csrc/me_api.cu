@@ -196,6 +196,20 @@ int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sig
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 
+int ga_uncertainty(const float* obs, int64_t N, const uint8_t* mask, const float* sigma, const double* lambda_grid_A, int L,
+                   const me_line_data* line_data, const ga_cfg* cfg, const float* params, float* out_sigma, float* out_chi2,
+                   void* stream) {
+    me::SynthDesc sd; me::GaDesc gd;
+    int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
+    if (rc != ME_OK) return rc;
+    rc = build_ga_desc(cfg, sd.npar, sigma, L, 0, N, true, gd);
+    if (rc != ME_OK) return rc;
+    if (N == 0) return ME_OK;
+    if (obs == nullptr || params == nullptr || out_sigma == nullptr) return ME_ERR_NULL;
+    cudaError_t e = me::launch_uncertainty(sd, gd, obs, mask, cfg->mu, N, params, out_sigma, out_chi2, (cudaStream_t)stream);
+    return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
 int ga_fitness(const float* genes, const float* obs, int64_t N, const float* sigma, const double* lambda_grid_A, int L,
                const me_line_data* line_data, const ga_cfg* cfg, float* chi2_out, void* stream) {
     me::SynthDesc sd; me::GaDesc gd;

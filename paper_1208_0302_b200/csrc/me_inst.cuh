@@ -13,12 +13,8 @@ namespace me {
 // nm_s:  shared memory, per wavelength pair one float2 of I_fixed (M = 11 only).
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET, int M>
-__device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
-                                         const float4* obs_s, const float2* nm_s, const float* pix) {
-    float p[M];
-#pragma unroll
-    for (int j = 0; j < M; ++j) p[j] = decode_gene(gene_value(g[j], gd), gd, j);
-    if (!gd.log_scale[1]) p[1] = fmaf(pix[5], gene_value(g[1], gd), pix[4]);   // inclination: per-pixel box (reading P1)
+__device__ __forceinline__ float fitness_params(const float* p, float mu, const SynthDesc& sd, const GaDesc& gd,
+                                                const float4* obs_s, const float2* nm_s, const float* pix) {
     Individual<NL> ind;
     setup_individual<NL, M>(ind, p, mu, sd);
     f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
@@ -43,6 +39,18 @@ __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDe
     float chi2 = gd.inv_nu * fmaf(pw[0], sI, fmaf(pw[1], sQ, fmaf(pw[2], sU, pw[3] * sV)));
     if (!(chi2 < __int_as_float(0x7f800000))) chi2 = __int_as_float(0x7f800000);   // NaN / Inf -> +Inf (reading G4)
     return chi2;
+}
+
+// Fitness of one individual held in registers as genes: decode (readings G1 / V0; inclination on the per-pixel box,
+// reading P1) -> fitness_params.
+template <int NL, bool TRIPLET, int M>
+__device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
+                                         const float4* obs_s, const float2* nm_s, const float* pix) {
+    float p[M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) p[j] = decode_gene(gene_value(g[j], gd), gd, j);
+    if (!gd.log_scale[1]) p[1] = fmaf(pix[5], gene_value(g[1], gd), pix[4]);   // inclination: per-pixel box (reading P1)
+    return fitness_params<NL, TRIPLET, M>(p, mu, sd, gd, obs_s, nm_s, pix);
 }
 
 // Stage I_fixed[L] pair-wise: nm_s[jp] = (F[2jp], F[2jp+1]); the odd tail duplicates its single value.
@@ -244,6 +252,143 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// ga_uncertainty: sigma of every parameter from the curvature of chi2 at the optimum (eq. 26; reading
+// U1 of DESIGN.md).  CTA = pixel.  The 1 + 2 (2M + 2M(M-1)) chi2 evaluations (325 for M = 9) of the central second
+// differences at h = 2^-7 and h/2 are spread over the block and run through the same fused fitness as the GA; thread 0
+// then builds the Richardson-extrapolated Hessian and inverts it in FP64 (Gauss-Jordan, partial pivoting; M <= 11).
+// Dynamic shared memory: scratch [64] | pix [8] | obs_s | nm_s | chi2v [n_eval]
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int unc_n_eval(int M) { return 1 + 2 * (2 * M + 2 * M * (M - 1)); }
+
+// offsets of evaluation e (same list as the specification): returns the step and the (at most two) displaced coordinates
+__device__ __forceinline__ void unc_offsets(int M, int e, float h, int& j, float& dj, int& k, float& dk) {
+    j = k = -1; dj = dk = 0.f;
+    if (e == 0) return;
+    const int per_level = 2 * M + 2 * M * (M - 1);
+    int r = e - 1;
+    const int level = r / per_level;
+    r -= level * per_level;
+    const float hl = level == 0 ? h : 0.5f * h;
+    if (r < 2 * M) { j = r >> 1; dj = (r & 1) ? -hl : hl; return; }
+    r -= 2 * M;
+    int pair = r >> 2;
+    const int q = r & 3;
+    j = 0;
+    while (pair >= M - 1 - j) { pair -= M - 1 - j; ++j; }
+    k = j + 1 + pair;
+    dj = (q < 2) ? hl : -hl;
+    dk = (q & 1) ? -hl : hl;
+}
+
+template <int NL, bool TRIPLET, int M>
+__global__ void __launch_bounds__(128, 4)
+ga_uncertainty_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
+                      const float* __restrict__ obs, const uint8_t* __restrict__ mask, const float* __restrict__ mu_arr,
+                      int64_t N, const float* __restrict__ params, float* __restrict__ out_sigma, float* __restrict__ out_chi2) {
+    extern __shared__ float4 smem4[];
+    const int L = sd.L, tid = threadIdx.x;
+    uint32_t* scratch = reinterpret_cast<uint32_t*>(smem4);
+    float* pix_s = reinterpret_cast<float*>(scratch + 64);
+    float* obs_s = pix_s + ME_PIX_WORDS;
+    float2* nm_s = reinterpret_cast<float2*>(obs_s + 8 * ((L + 1) >> 1));
+    float* chi2v = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));
+    if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, tid, 128);
+    const int ne = unc_n_eval(M);
+    const float h = 1.0f / 128.0f;
+    const float qnan = __int_as_float(0x7fc00000);
+    for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
+        if (mask != nullptr && mask[n] == 0) {
+            if (tid < M) out_sigma[n * M + tid] = qnan;
+            if (tid == 0 && out_chi2 != nullptr) out_chi2[n] = qnan;
+            continue;
+        }
+        const float mu = mu_arr != nullptr ? __ldg(mu_arr + n) : 1.0f;
+        __syncthreads();
+        stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, 128);
+        __syncthreads();
+        pixel_prologue(obs_s, L, gd, pix_s, tid == 0);
+        __syncthreads();
+        // box coordinates of the optimum (inverse of the decode of reading G1; inclination on the per-pixel box)
+        float u0[M], lo[M], span[M];
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            const float pj = __ldg(params + n * M + j);
+            lo[j] = gd.lo[j]; span[j] = gd.log_scale[j] ? gd.log2ratio[j] : gd.span[j];
+            if (j == 1 && !gd.log_scale[1]) { lo[j] = pix_s[4]; span[j] = pix_s[5]; }
+            if (gd.log_scale[j]) u0[j] = span[j] != 0.f ? log2f(pj / lo[j]) / span[j] : 0.f;
+            else u0[j] = span[j] != 0.f ? (pj - lo[j]) / span[j] : 0.f;
+        }
+        for (int e = tid; e < ne; e += 128) {
+            int j1, j2; float d1, d2;
+            unc_offsets(M, e, h, j1, d1, j2, d2);
+            float p[M];
+#pragma unroll
+            for (int j = 0; j < M; ++j) {
+                const float u = u0[j] + (j == j1 ? d1 : 0.f) + (j == j2 ? d2 : 0.f);
+                p[j] = gd.log_scale[j] ? lo[j] * exp2f(u * span[j]) : fmaf(span[j], u, lo[j]);
+            }
+            chi2v[e] = fitness_params<NL, TRIPLET, M>(p, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s);
+        }
+        __syncthreads();
+        if (tid == 0) {
+            const int per_level = 2 * M + 2 * M * (M - 1);
+            double H[M * M], Vn[M * M];
+            int idx[M], na = 0;
+            for (int j = 0; j < M; ++j) if (span[j] != 0.f) idx[na++] = j;
+            const double c0 = (double)chi2v[0];
+            for (int a = 0; a < na; ++a)
+                for (int b = a; b < na; ++b) {
+                    const int j = idx[a], k = idx[b];
+                    double D[2];
+                    for (int level = 0; level < 2; ++level) {
+                        const double hl = level == 0 ? (double)h : 0.5 * (double)h;
+                        const float* c = chi2v + 1 + level * per_level;
+                        if (j == k) D[level] = ((double)c[2 * j] - 2.0 * c0 + (double)c[2 * j + 1]) / (hl * hl);
+                        else {
+                            int pair = 0;
+                            for (int q = 0; q < j; ++q) pair += M - 1 - q;
+                            pair += k - j - 1;
+                            const float* q4 = c + 2 * M + 4 * pair;
+                            D[level] = ((double)q4[0] - (double)q4[1] - (double)q4[2] + (double)q4[3]) / (4.0 * hl * hl);
+                        }
+                    }
+                    H[a * na + b] = H[b * na + a] = (4.0 * D[1] - D[0]) / 3.0;      // Richardson / Neville, one level
+                }
+            for (int a = 0; a < na; ++a) for (int b = 0; b < na; ++b) Vn[a * na + b] = a == b ? 1.0 : 0.0;
+            bool ok = na > 0;
+            for (int c = 0; c < na && ok; ++c) {                                     // Gauss-Jordan, partial pivoting
+                int piv = c;
+                for (int r = c + 1; r < na; ++r) if (fabs(H[r * na + c]) > fabs(H[piv * na + c])) piv = r;
+                if (!(fabs(H[piv * na + c]) > 0.0)) { ok = false; break; }
+                for (int q = 0; q < na; ++q) {
+                    double t = H[c * na + q]; H[c * na + q] = H[piv * na + q]; H[piv * na + q] = t;
+                    t = Vn[c * na + q]; Vn[c * na + q] = Vn[piv * na + q]; Vn[piv * na + q] = t;
+                }
+                const double d = 1.0 / H[c * na + c];
+                for (int q = 0; q < na; ++q) { H[c * na + q] *= d; Vn[c * na + q] *= d; }
+                for (int r = 0; r < na; ++r) {
+                    if (r == c) continue;
+                    const double f = H[r * na + c];
+                    if (f == 0.0) continue;
+                    for (int q = 0; q < na; ++q) { H[r * na + q] -= f * H[c * na + q]; Vn[r * na + q] -= f * Vn[c * na + q]; }
+                }
+            }
+            for (int a = 0; a < na && ok; ++a) if (!(Vn[a * na + a] > 0.0)) ok = false;
+            for (int j = 0; j < M; ++j) out_sigma[n * M + j] = span[j] != 0.f ? qnan : 0.f;
+            if (ok)
+                for (int a = 0; a < na; ++a) {
+                    const int j = idx[a];
+                    const double su = sqrt(Vn[a * na + a] * c0 / M);                 // eq. 26
+                    const double dpdu = gd.log_scale[j] ? (double)__ldg(params + n * M + j) * 0.6931471805599453 * (double)span[j]
+                                                        : (double)span[j];
+                    out_sigma[n * M + j] = (float)(su * fabs(dpdu));
+                }
+            if (out_chi2 != nullptr) out_chi2[n] = chi2v[0];
+        }
+    }
+}
+
 // Test hook: the fused fitness alone (128 threads per pixel, individuals strided over the block).
 template <int NL, bool TRIPLET, int M>
 __global__ void __launch_bounds__(128, 4)
@@ -313,6 +458,15 @@ cudaError_t ME_INST_NAME(launch_ga_fitness)(const SynthDesc& sd, const GaDesc& g
                                             const float* mu, int64_t N, float* chi2_out, cudaStream_t st) {
     const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + ME_PIX_WORDS * 4;
     ga_fitness_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid_for_(N), 128, smem, st>>>(sd, gd, genes, obs, mu, N, chi2_out);
+    return cudaGetLastError();
+}
+
+cudaError_t ME_INST_NAME(launch_uncertainty)(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask,
+                                             const float* mu, int64_t N, const float* params, float* out_sigma,
+                                             float* out_chi2, cudaStream_t st) {
+    const size_t smem = 64 * 4 + ME_PIX_WORDS * 4 + (size_t)40 * ((sd.L + 1) / 2) + (size_t)4 * (1 + 2 * (2 * ME_INST_M + 2 * ME_INST_M * (ME_INST_M - 1)));
+    ga_uncertainty_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid_for_(N), 128, smem, st>>>(sd, gd, obs, mask, mu, N, params,
+                                                                                                  out_sigma, out_chi2);
     return cudaGetLastError();
 }
 

@@ -119,6 +119,8 @@ static inline unsigned grid_for(int64_t n) { return (unsigned)(n < 0x7fffffffLL 
                                                     int64_t, float*, float*, cudaStream_t);                                     \
     cudaError_t launch_ga_fitness_##NL##_##TAG##_##M(const SynthDesc&, const GaDesc&, const float*, const float*, const float*,  \
                                                      int64_t, float*, cudaStream_t);                                            \
+    cudaError_t launch_uncertainty_##NL##_##TAG##_##M(const SynthDesc&, const GaDesc&, const float*, const uint8_t*,           \
+                                                      const float*, int64_t, const float*, float*, float*, cudaStream_t);        \
     cudaError_t launch_synth_##NL##_##TAG##_##M(const SynthDesc&, const float*, const float*, int64_t, float*, const float*,    \
                                                 const float*, float, float*, cudaStream_t);
 ME_DECL_INST(1, t, 9) ME_DECL_INST(2, t, 9) ME_DECL_INST(4, t, 9) ME_DECL_INST(1, g, 9) ME_DECL_INST(2, g, 9) ME_DECL_INST(4, g, 9)
@@ -144,6 +146,11 @@ ME_DECL_INST(1, t, 11) ME_DECL_INST(2, t, 11) ME_DECL_INST(4, t, 11) ME_DECL_INS
 cudaError_t launch_ga_invert(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask, const float* mu,
                              int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
     ME_DISPATCH(launch_ga_invert, sd, gd, obs, mask, mu, N, out_params, out_chi2, st);
+}
+
+cudaError_t launch_uncertainty(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask, const float* mu,
+                               int64_t N, const float* params, float* out_sigma, float* out_chi2, cudaStream_t st) {
+    ME_DISPATCH(launch_uncertainty, sd, gd, obs, mask, mu, N, params, out_sigma, out_chi2, st);
 }
 
 cudaError_t launch_ga_fitness(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs, const float* mu,

@@ -10,6 +10,8 @@ struct GaDesc;
 
 cudaError_t launch_ga_invert(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask, const float* mu,
                              int64_t N, float* out_params, float* out_chi2, cudaStream_t st);
+cudaError_t launch_uncertainty(const SynthDesc& sd, const GaDesc& gd, const float* obs, const uint8_t* mask, const float* mu,
+                               int64_t N, const float* params, float* out_sigma, float* out_chi2, cudaStream_t st);
 cudaError_t launch_ga_fitness(const SynthDesc& sd, const GaDesc& gd, const float* genes, const float* obs, const float* mu,
                               int64_t N, float* chi2_out, cudaStream_t st);
 cudaError_t launch_ga_step(const GaDesc& gd, int npar, const float* genes_in, const float* chi2_in, int64_t N, int t,
