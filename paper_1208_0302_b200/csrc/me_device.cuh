@@ -164,6 +164,23 @@ MEDEV void faddeeva_far_acc(f2 v, f2 r2, const FarCoef& c, f2& sr, f2& si) {
     si = fma2(mul2(v, r), Y, si);
 }
 
+// The same coefficients parked in shared memory (one float4 pair per thread and line) and re-loaded inside the far branch:
+// in registers they do not fit next to the fitness loop's working set and the compiler rematerialises them with ~13
+// scalar FMULs per line and pair on the FMA pipe (profiles/r1e); an LDS.128 pair costs no FMA-pipe slot.
+MEDEV FarCoef far_load(const float4* p, int stride) {
+    float4 x, y;
+    const unsigned ax = (unsigned)__cvta_generic_to_shared(p), ay = (unsigned)__cvta_generic_to_shared(p + stride);
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(ax));
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(y.x), "=f"(y.y), "=f"(y.z), "=f"(y.w) : "r"(ay));
+    FarCoef c;
+    c.x3 = x.x; c.x2 = x.y; c.x1 = x.z; c.x0 = x.w; c.y3 = y.x; c.y2 = y.y; c.y1 = y.z; c.y0 = y.w;
+    return c;
+}
+MEDEV void far_store(float4* p, int stride, const FarCoef& c) {
+    p[0] = make_float4(c.x3, c.x2, c.x1, c.x0);
+    p[stride] = make_float4(c.y3, c.y2, c.y1, c.y0);
+}
+
 // Core region (Weideman).  D = 1/(L - iz) = r ((L+a) + i v), r = 1/|L - iz|^2, Z = (L + iz) D.  With t = 2 Re Z,
 // m = -|Z|^2 the recurrence gives p(Z) = b0 - b1 conj(Z), and conj(Z) D = r conj(L + iz), so
 //   p D = r [ (b0 (L+a) - b1 (L-a)) + i v (b0 + b1) ],     w = D (p D + 1/sqrt(pi)).
@@ -204,6 +221,8 @@ struct Individual {
     float c2x, s2x;                   // cos 2chi, sin 2chi
     float S0, muS1;                   // 11-parameter model: (1-s) S0 and (1-s) alpha mu S1
     float k0, nmS1, stray;            // 11-parameter model only: eta0/sqrt(pi), (1-s)(1-alpha) mu S1, s
+    float4* far_s;                    // FARS: this thread's far coefficients in shared memory, [2 l + {0,1}] * far_stride
+    int far_stride;
 };
 
 // p: decoded parameter vector, M = 9 or 11 entries.  For M = 11 (reading F13)
@@ -246,9 +265,9 @@ MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const
 
 // Profile sums of one line at a pair of reduced wavelengths v:
 //   S_kind += r_l * sum_c weight_c * w(v - shift_c vB + i a)
-template <bool TRIPLET>
-MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far, float far2, const SynthDesc& d, int l,
-                         f2& br, f2& bi, f2& pr, f2& pi, f2& rr, f2& ri) {
+template <bool TRIPLET, bool FARS>
+MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far_r, const float4* far_s, int far_stride,
+                         float far2, const SynthDesc& d, int l, f2& br, f2& bi, f2& pr, f2& pi, f2& rr, f2& ri) {
     const float r = d.line[l].strength;
     if (TRIPLET) {
         const float gvB = d.line[l].g * vB;
@@ -259,6 +278,7 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
         // When all six arguments lie in one wing tier (the common case) the three evaluations are independent
         // straight-line code that the scheduler interleaves; the series shortens with distance from the line.
         if (rmin >= far2) {
+            const FarCoef far = FARS ? far_load(far_s + 2 * l * far_stride, far_stride) : far_r;
             faddeeva_far_acc(v, r2p, far, pr, pi);
             faddeeva_far_acc(vb, r2b, far, br, bi);
             faddeeva_far_acc(vr, r2r, far, rr, ri);
@@ -306,7 +326,7 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
 // The Unno-Rachkovsky solution is evaluated in the frame chi = 0 (eta_U = rho_U = 0) and Q,U are rotated by 2 chi.
 // M = 11: nmF = I_fixed at the two wavelengths; the field-free profile sum phi_nm = sum_l r_l H(a, v_l) is the pi sum of
 // effective triplets (their pi component is unshifted with weight 1), else one extra Voigt per line.
-template <int NL, bool TRIPLET, int M>
+template <int NL, bool TRIPLET, int M, bool FARS = false>
 MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2 nmF, f2& I, f2& Q, f2& U, f2& V) {
     f2 br = bc(0.f), bi = bc(0.f), pr = bc(0.f), pi = bc(0.f), rr = bc(0.f), ri = bc(0.f), nr = bc(0.f);
 #pragma unroll
@@ -314,7 +334,8 @@ MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bo
         if (NL == ME_MAX_LINES && l >= d.n_lines) break;      // NL == ME_MAX_LINES is the run-time-sized fallback
         const f2 off = tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]);
         const f2 v = fma2(ind.invD[l], off, ind.v0[l]);
-        line_profiles<TRIPLET>(v, ind.vB[l], ind.fad, ind.far[l], ind.far2, d, l, br, bi, pr, pi, rr, ri);
+        line_profiles<TRIPLET, FARS>(v, ind.vB[l], ind.fad, ind.far[l], ind.far_s, ind.far_stride, ind.far2, d, l, br, bi,
+                                     pr, pi, rr, ri);
         if (M == ME_MAX_NPAR && !TRIPLET) {
             f2 wr, wi;
             faddeeva_pair(v, ind.fad, wr, wi);

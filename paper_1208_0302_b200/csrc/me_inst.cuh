@@ -12,16 +12,23 @@ namespace me {
 // obs_s: shared memory, per wavelength pair two float4 = (I0,I1,Q0,Q1), (U0,U1,V0,V1) (broadcast reads, conflict-free).
 // nm_s:  shared memory, per wavelength pair one float2 of I_fixed (M = 11 only).
 // ------------------------------------------------------------------------------------------------------------
-template <int NL, bool TRIPLET, int M>
+// far_s != nullptr (FARS): [2 NL][far_stride] float4 of shared memory, this thread's column.
+template <int NL, bool TRIPLET, int M, bool FARS = false>
 __device__ __forceinline__ float fitness_params(const float* p, float mu, const SynthDesc& sd, const GaDesc& gd,
-                                                const float4* obs_s, const float2* nm_s, const float* pix) {
+                                                const float4* obs_s, const float2* nm_s, const float* pix,
+                                                float4* far_s = nullptr, int far_stride = 0) {
     Individual<NL> ind;
     setup_individual<NL, M>(ind, p, mu, sd);
+    ind.far_s = far_s; ind.far_stride = far_stride;
+    if (FARS) {
+#pragma unroll
+        for (int l = 0; l < NL; ++l) far_store(far_s + 2 * l * far_stride, far_stride, ind.far[l]);
+    }
     f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
     const int L = sd.L, npair = L >> 1;
     for (int jp = 0; jp < npair; ++jp) {
         f2 I, Q, U, V;
-        stokes_pair<NL, TRIPLET, M>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V);
+        stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V);
         const float4 o0 = obs_s[2 * jp], o1 = obs_s[2 * jp + 1];           // (I0,I1,Q0,Q1), (U0,U1,V0,V1)
         const f2 dI = sub2(make_float2(o0.x, o0.y), I), dQ = sub2(make_float2(o0.z, o0.w), Q);
         const f2 dU = sub2(make_float2(o1.x, o1.y), U), dV = sub2(make_float2(o1.z, o1.w), V);
@@ -29,7 +36,7 @@ __device__ __forceinline__ float fitness_params(const float* p, float mu, const 
     }
     if (L & 1) {                                                            // odd tail: second half is a duplicate, dropped
         f2 I, Q, U, V;
-        stokes_pair<NL, TRIPLET, M>(ind, sd, L - 1, true, M == ME_MAX_NPAR ? nm_s[npair] : bc(0.f), I, Q, U, V);
+        stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, L - 1, true, M == ME_MAX_NPAR ? nm_s[npair] : bc(0.f), I, Q, U, V);
         const float4 o0 = obs_s[2 * npair], o1 = obs_s[2 * npair + 1];
         const float dI = o0.x - I.x, dQ = o0.z - Q.x, dU = o1.x - U.x, dV = o1.z - V.x;
         aI.x = fmaf(dI, dI, aI.x); aQ.x = fmaf(dQ, dQ, aQ.x); aU.x = fmaf(dU, dU, aU.x); aV.x = fmaf(dV, dV, aV.x);
@@ -43,14 +50,15 @@ __device__ __forceinline__ float fitness_params(const float* p, float mu, const 
 
 // Fitness of one individual held in registers as genes: decode (readings G1 / V0; inclination on the per-pixel box,
 // reading P1) -> fitness_params.
-template <int NL, bool TRIPLET, int M>
+template <int NL, bool TRIPLET, int M, bool FARS = false>
 __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
-                                         const float4* obs_s, const float2* nm_s, const float* pix) {
+                                         const float4* obs_s, const float2* nm_s, const float* pix,
+                                         float4* far_s = nullptr, int far_stride = 0) {
     float p[M];
 #pragma unroll
     for (int j = 0; j < M; ++j) p[j] = decode_gene(gene_value(g[j], gd), gd, j);
     if (!gd.log_scale[1]) p[1] = fmaf(pix[5], gene_value(g[1], gd), pix[4]);   // inclination: per-pixel box (reading P1)
-    return fitness_params<NL, TRIPLET, M>(p, mu, sd, gd, obs_s, nm_s, pix);
+    return fitness_params<NL, TRIPLET, M, FARS>(p, mu, sd, gd, obs_s, nm_s, pix, far_s, far_stride);
 }
 
 // Stage I_fixed[L] pair-wise: nm_s[jp] = (F[2jp], F[2jp+1]); the odd tail duplicates its single value.
@@ -63,7 +71,8 @@ __device__ __forceinline__ void stage_nm(float2* nm_s, const float* nm, int L, i
 
 // ------------------------------------------------------------------------------------------------------------
 // The fused GA inversion kernel.
-// Dynamic shared memory: scratch [64] | pix [8] (per-pixel weights and inclination box) | obs_s [ceil(L/2)] 2 x float4 |
+// Dynamic shared memory: scratch [64] | pix [8] (per-pixel weights and inclination box) | far [2 NL][THREADS] float4
+//                        (far-tier coefficients of every thread) | obs_s [ceil(L/2)] 2 x float4 |
 //                        nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] | order [pop] u16 (variant 1: ranks at restarts)
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET, int M, int THREADS, int MINB>
@@ -76,7 +85,9 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
     // fixed offsets first (compile-time shared addresses, no pointer registers): scratch [64] | pix [8] | obs_s ...
     uint32_t* scratch = reinterpret_cast<uint32_t*>(smem4);
     float* pix_s = reinterpret_cast<float*>(scratch + 64);
-    float* obs_s = pix_s + ME_PIX_WORDS;
+    constexpr bool FARS = TRIPLET && NL <= 2;                  // far-tier coefficients parked in shared memory
+    float4* far_s = reinterpret_cast<float4*>(pix_s + ME_PIX_WORDS) + threadIdx.x;   // [2 NL][THREADS] float4, own column
+    float* obs_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? 2 * NL * THREADS : 0));
     float2* nm_s = reinterpret_cast<float2*>(obs_s + 8 * ((L + 1) >> 1));
     float* genes_s = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));
     float* chi2_s = genes_s + 2 * pop * M;
@@ -133,7 +144,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
                 } else {
                     make_child<M>(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
                 }
-                if (evaluate) f = fitness<NL, TRIPLET, M>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s);
+                if (evaluate) f = fitness<NL, TRIPLET, M, FARS>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s, far_s, THREADS);
 #pragma unroll
                 for (int j = 0; j < M; ++j) gnext[tid * M + j] = g[j];
                 chi2_s[(cur ^ 1) * pop + tid] = f;
@@ -427,7 +438,8 @@ static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, con
                                       const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
     auto k = ga_invert_kernel<NL, TRIPLET, M, THREADS, MINB>;
     const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * M * 4 + (size_t)2 * gd.pop * 4 + 64 * 4 +
-                        (size_t)2 * gd.pop + 16 + ME_PIX_WORDS * 4;
+                        (size_t)2 * gd.pop + 16 + ME_PIX_WORDS * 4 +
+                        ((TRIPLET && NL <= 2) ? (size_t)2 * NL * THREADS * 16 : 0);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid_for_(N), THREADS, smem, st>>>(sd, gd, obs, mask, mu, N, out_params, out_chi2);
