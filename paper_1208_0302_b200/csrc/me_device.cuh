@@ -110,7 +110,9 @@ MEDEV FadConst fad_const(float a) {
 
 // Wing region.  With t = 2 Re q, m = -|q|^2 the recurrence gives R(q) = b0 - b1 conj(q); since s conj(q) = |s|^2 conj(s)
 // and |s|^2 = r = 1/|z|^2:   w = i s R = r [ a (b0 + r b1) + i v (b0 - r b1) ]   (no cancellation in H).
-// K = number of series terms beyond the leading one: 5 for |z| >= FAD_CUT, 3 for >= FAD_MID, 2 for >= FAD_FAR.
+// K = number of series terms beyond the leading one: 5 for |z| >= FAD_CUT, 2 for >= FAD_FAR (used as written only when
+// a > FAD_FAR_AMAX; otherwise the far tier below).  An intermediate K = 3 tier (|z| >= 7.5) was measured and dropped: it
+// saved 0.7 % of the arithmetic and cost more than that in code size (profiles/r1e).
 template <int K>
 MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
     const f2 r = rcp2(r2);                                    // 1/|z|^2
@@ -288,10 +290,6 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
             faddeeva_wing<2>(v, r2p, fad, w0r, w0i);
             faddeeva_wing<2>(vb, r2b, fad, w1r, w1i);
             faddeeva_wing<2>(vr, r2r, fad, w2r, w2i);
-        } else if (rmin >= FAD_MID2) {
-            faddeeva_wing<3>(v, r2p, fad, w0r, w0i);
-            faddeeva_wing<3>(vb, r2b, fad, w1r, w1i);
-            faddeeva_wing<3>(vr, r2r, fad, w2r, w2i);
         } else if (rmin >= FAD_CUT2) {
             faddeeva_wing<5>(v, r2p, fad, w0r, w0i);
             faddeeva_wing<5>(vb, r2b, fad, w1r, w1i);
