@@ -44,10 +44,20 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-aux", action="store_true", help="skip the auxiliary me_synth (config2) measurement")
+    ap.add_argument("--zeeman", default="triplets", choices=["triplets", "full"],
+                    help="full = LS-coupling Zeeman patterns (12 + 3 components, PAPER.md:351) instead of effective triplets; "
+                         "a measured variant, not the headline configuration")
     return ap.parse_args()
 
 
 def workload(args):
+    c, n, side = _workload(args)
+    if getattr(args, "zeeman", "triplets") == "full":
+        c = dict(c, triplets=False)
+    return c, n, side
+
+
+def _workload(args):
     if args.workload == "config0":
         c = W.config0()
         return c, c["n_pixels"], None
@@ -117,8 +127,13 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------ oracle legs
 def oracle_lines_for(cfg):
     from oracle import api as orc
-    lines = [dict(lambda0=l["lambda0"], strength=l["strength"], shift=[0.0, -l["g_eff"], l["g_eff"]], weight=[1, 1, 1],
-                  kind=[0, -1, 1]) for l in cfg["lines"]]
+    lines = []
+    for l in cfg["lines"]:
+        if cfg["triplets"]:
+            sh, we, ki = [0.0, -l["g_eff"], l["g_eff"]], [1, 1, 1], [0, -1, 1]
+        else:
+            sh, we, ki = orc.zeeman_pattern(l["lower"], l["upper"])
+        lines.append(dict(lambda0=l["lambda0"], strength=l["strength"], shift=sh, weight=we, kind=ki))
     return orc.Lines(lines, W.LAMBDA_REF)
 
 
@@ -358,7 +373,7 @@ def run_b200(args):
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg["name"], "pixels_per_gpu": n_pixels, "active_pixels_per_gpu": n_active, "L": L,
                        "pop": ga["pop"], "generations": ga["generations"], "lines": len(cfg["lines"]),
-                       "zeeman": "effective triplets", "parallelism": "pixel shards x%d" % world,
+                       "zeeman": "effective triplets" if cfg["triplets"] else "full LS patterns", "parallelism": "pixel shards x%d" % world,
                        "l2": "obs cube %.0f MB per step (> 126 MB L2 for config1/3); path is ALU-bound" % (obs.numel() * 4 / 1e6)},
             "syntheses_per_s": value * syn, "median_chi2": med_chi2,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,

@@ -56,6 +56,8 @@ int build_synth_desc(const double* lambda, int L, const me_line_data* ld, me::Sy
         q.triplet = (cnt[0] == 1 && cnt[1] == 1 && cnt[2] == 1 && d.weight[b] == 1.0f && d.weight[p] == 1.0f &&
                      d.weight[r] == 1.0f && d.shift[p] == 0.0f && d.shift[b] == -d.shift[r]) ? 1 : 0;
         q.g = q.triplet ? d.shift[r] : 0.0f;
+        q.smax = 0.0f;
+        for (int c = q.kind_begin[0]; c < o; ++c) q.smax = std::fmax(q.smax, std::fabs(d.shift[c]));
         if (!q.triplet) d.all_triplets = 0;
         for (int j = 0; j < L; ++j) d.off[l][j] = (float)(lambda[j] - ln.lambda0_A);   // formed in double, rounded once
     }

@@ -28,7 +28,8 @@ struct LineDesc {
     int kind_begin[4];      // components sorted by kind: [blue | pi | red], kind_begin[3] = end
     int triplet;            // 1 if exactly one component per kind with weight 1 and shifts (-g, 0, +g)
     float g;                // Lande factor of the triplet
-    int pad[2];
+    float smax;             // largest |shift| of the line's components (outermost Zeeman component, Lorentz units)
+    int pad;
 };
 
 struct alignas(16) SynthDesc {
@@ -303,18 +304,42 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
         br = fma2(r, w1r, br); bi = fma2(r, w1i, bi);
         rr = fma2(r, w2r, rr); ri = fma2(r, w2i, ri);
     } else {
+        // General component list (full Zeeman patterns).  Every component sits within smax |vB| of the
+        // line centre, so the smallest |z|^2 over all of them and both wavelengths is bounded below by
+        // (max(0, min|v| - smax |vB|))^2 + a^2: one tier for the whole line, chosen without touching the components.
         const int* kb = d.line[l].kind_begin;
-        for (int c = kb[0]; c < kb[1]; ++c) {
-            f2 wr, wi; faddeeva_pair(add2(v, bc(-d.shift[c] * vB)), fad, wr, wi);
-            const float s = r * d.weight[c]; br = fma2(s, wr, br); bi = fma2(s, wi, bi);
-        }
-        for (int c = kb[1]; c < kb[2]; ++c) {
-            f2 wr, wi; faddeeva_pair(add2(v, bc(-d.shift[c] * vB)), fad, wr, wi);
-            const float s = r * d.weight[c]; pr = fma2(s, wr, pr); pi = fma2(s, wi, pi);
-        }
-        for (int c = kb[2]; c < kb[3]; ++c) {
-            f2 wr, wi; faddeeva_pair(add2(v, bc(-d.shift[c] * vB)), fad, wr, wi);
-            const float s = r * d.weight[c]; rr = fma2(s, wr, rr); ri = fma2(s, wi, ri);
+        const float dmin = fmaxf(fminf(fabsf(v.x), fabsf(v.y)) - d.line[l].smax * fabsf(vB), 0.0f);
+        const float rmin = fmaf(dmin, dmin, fad.a2);
+        const FarCoef far = far_r;
+        const int tier = rmin >= far2 ? 2 : (rmin >= FAD_CUT2 ? 1 : 0);
+#pragma unroll 1
+        for (int k = 0; k < 3; ++k) {                              // k = 0 blue, 1 pi, 2 red
+            f2 ar = bc(0.f), ai = bc(0.f);
+            if (tier == 2) {
+                for (int c = kb[k]; c < kb[k + 1]; ++c) {
+                    const f2 vc = add2(v, bc(-d.shift[c] * vB));
+                    const f2 rr_ = rcp2(fma2(vc, vc, fad.a2));                        // 1 / |z|^2
+                    const f2 rw = mul2(d.weight[c], rr_);                             // weight_c / |z|^2
+                    const f2 X = fma2(fma2(fma2(bc(far.x3), rr_, far.x2), rr_, far.x1), rr_, far.x0);
+                    const f2 Y = fma2(fma2(fma2(bc(far.y3), rr_, far.y2), rr_, far.y1), rr_, far.y0);
+                    ar = fma2(rw, X, ar);
+                    ai = fma2(mul2(vc, rw), Y, ai);
+                }
+            } else if (tier == 1) {
+                for (int c = kb[k]; c < kb[k + 1]; ++c) {
+                    const f2 vc = add2(v, bc(-d.shift[c] * vB));
+                    f2 wr, wi; faddeeva_wing<5>(vc, fma2(vc, vc, fad.a2), fad, wr, wi);
+                    const float sw = r * d.weight[c]; ar = fma2(sw, wr, ar); ai = fma2(sw, wi, ai);
+                }
+            } else {
+                for (int c = kb[k]; c < kb[k + 1]; ++c) {
+                    f2 wr, wi; faddeeva_pair(add2(v, bc(-d.shift[c] * vB)), fad, wr, wi);
+                    const float sw = r * d.weight[c]; ar = fma2(sw, wr, ar); ai = fma2(sw, wi, ai);
+                }
+            }
+            if (k == 0) { br = add2(br, ar); bi = add2(bi, ai); }
+            else if (k == 1) { pr = add2(pr, ar); pi = add2(pi, ai); }
+            else { rr = add2(rr, ar); ri = add2(ri, ai); }
         }
     }
 }
