@@ -245,3 +245,30 @@ def test_config3_full_size_sampled_parity(B):
     chi_o = np.array(chi_o)
     assert np.all(np.abs(gc_h[idx] - chi_o) <= 0.25 * chi_o)
     assert np.mean(np.abs(gc_h[idx] - chi_o) <= 2e-4 * chi_o) >= 0.75
+
+
+def test_maximum_sizes(B):
+    # the largest population (ME_MAX_POP = 1024 -> 1024-thread CTAs) on the longest grid (ME_MAX_L = 512), two lines,
+    # and the largest generation count the ABI accepts (schedule table of ME_MAX_GEN + 1 entries) on a cheap problem
+    lines, lam = [W.FE_6301, W.FE_6302], W.grid(6302.0, 512, 0.006)
+    cfgw = dict(lines=lines, triplets=True, lam=lam, sigma=1e-3, b_range=(10.0, 3000.0))
+    N = 2
+    truth, obs, ln = make_obs(cfgw, N, threads=NTHREADS)
+    ga = W.ga_config(1024, 2)
+    res = orc.ga_invert(obs, lam, ln, ga, seed=4, threads=NTHREADS)
+    ld = B.line_data_from_workload(lines, True)
+    gp, gc = B.ga_invert(dev(obs), lam, ld, ga, 4)
+    assert np.max(np.abs(gc.cpu().numpy() - res["chi2"]) / res["chi2"]) < 2e-4
+    assert np.allclose(gp.cpu().numpy(), res["params"], rtol=1e-4, atol=1e-4)
+    c0 = W.config0()
+    t0, o0, l0 = make_obs(c0, 3, threads=NTHREADS)
+    gmax = W.ga_config(8, 1023)
+    r0 = orc.ga_invert(o0, c0["lam"], l0, gmax, seed=6, threads=3)
+    g0 = B.ga_invert(dev(o0), c0["lam"], B.line_data_from_workload(c0["lines"], True), gmax, 6)
+    assert np.max(np.abs(g0[1].cpu().numpy() - r0["chi2"]) / r0["chi2"]) < 0.05      # 1023 generations of trajectory
+    # one past the limits is refused, nothing is launched
+    for bad in (W.ga_config(1025, 2), W.ga_config(8, 1024)):
+        with pytest.raises(B.MeError):
+            B.ga_invert(dev(o0), c0["lam"], B.line_data_from_workload(c0["lines"], True), bad, 6)
+    with pytest.raises(B.MeError):
+        B.me_synth(dev(t0), W.grid(6302.5, 513, 0.01), B.line_data_from_workload(c0["lines"], True))
