@@ -350,12 +350,13 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
 // M = 11: nmF = I_fixed at the two wavelengths; the field-free profile sum phi_nm = sum_l r_l H(a, v_l) is the pi sum of
 // effective triplets (their pi component is unshifted with weight 1), else one extra Voigt per line.
 template <int NL, bool TRIPLET, int M, bool FARS = false>
-MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2 nmF, f2& I, f2& Q, f2& U, f2& V) {
+MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2 nmF, f2& I, f2& Q, f2& U, f2& V,
+                       const f2* offp = nullptr) {
     f2 br = bc(0.f), bi = bc(0.f), pr = bc(0.f), pi = bc(0.f), rr = bc(0.f), ri = bc(0.f), nr = bc(0.f);
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
         if (NL == ME_MAX_LINES && l >= d.n_lines) break;      // NL == ME_MAX_LINES is the run-time-sized fallback
-        const f2 off = tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]);
+        const f2 off = offp != nullptr ? offp[l] : (tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]));
         const f2 v = fma2(ind.invD[l], off, ind.v0[l]);
         line_profiles<TRIPLET, FARS>(v, ind.vB[l], ind.fad, ind.far[l], ind.far_s, ind.far_stride, ind.far2, d, l, br, bi,
                                      pr, pi, rr, ri);

@@ -26,9 +26,17 @@ __device__ __forceinline__ float fitness_params(const float* p, float mu, const 
     }
     f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
     const int L = sd.L, npair = L >> 1;
+    // the offsets lambda_j - lambda_l of the NEXT pair are loaded one iteration ahead: the indexed constant load otherwise
+    // stalls the first FFMA2 of every line (short scoreboard, profiles/r1e)
+    f2 offn[NL];
+#pragma unroll
+    for (int l = 0; l < NL; ++l) offn[l] = *reinterpret_cast<const f2*>(&sd.off[l][0]);
     for (int jp = 0; jp < npair; ++jp) {
-        f2 I, Q, U, V;
-        stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V);
+        f2 I, Q, U, V, offc[NL];
+        const int jn = 2 * min(jp + 1, npair - 1);
+#pragma unroll
+        for (int l = 0; l < NL; ++l) { offc[l] = offn[l]; offn[l] = *reinterpret_cast<const f2*>(&sd.off[l][jn]); }
+        stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V, offc);
         const float4 o0 = obs_s[2 * jp], o1 = obs_s[2 * jp + 1];           // (I0,I1,Q0,Q1), (U0,U1,V0,V1)
         const f2 dI = sub2(make_float2(o0.x, o0.y), I), dQ = sub2(make_float2(o0.z, o0.w), Q);
         const f2 dU = sub2(make_float2(o1.x, o1.y), U), dV = sub2(make_float2(o1.z, o1.w), V);
