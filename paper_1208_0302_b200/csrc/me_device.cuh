@@ -563,9 +563,22 @@ __device__ __forceinline__ void make_child(float* child, const float* genes, con
     }
 }
 
-// Stage obs[n] ([4][L] in HBM, rows contiguous => coalesced) into shared memory, pair-interleaved:
+// Stage obs[n] ([4][L] in HBM, rows contiguous) into shared memory, pair-interleaved:
 // element (s, j) -> word 8 (j/2) + 2 s + (j & 1).  Shared size: 8 * ceil(L/2) floats.
+// L % 4 == 0 (and a 16-byte aligned cube): one coalesced LDG.128 per thread (streaming, read once: no L1 allocation)
+// and two 8-byte shared stores; otherwise element-wise.
 __device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int L, int tid, int nthreads) {
+    if ((L & 3) == 0 && (reinterpret_cast<uintptr_t>(obs_n) & 15) == 0) {
+        for (int k4 = tid; k4 < L; k4 += nthreads) {
+            const int k = 4 * k4, s = k / L, j = k - s * L;     // the four values sit in one Stokes row (L % 4 == 0)
+            float4 x;
+            asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                         : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "l"(obs_n + k));
+            *reinterpret_cast<float2*>(obs_s + 8 * (j >> 1) + 2 * s) = make_float2(x.x, x.y);
+            *reinterpret_cast<float2*>(obs_s + 8 * ((j >> 1) + 1) + 2 * s) = make_float2(x.z, x.w);
+        }
+        return;
+    }
     for (int k = tid; k < 4 * L; k += nthreads) {
         const int s = k / L, j = k - s * L;
         obs_s[8 * (j >> 1) + 2 * s + (j & 1)] = __ldg(obs_n + k);
