@@ -28,6 +28,9 @@ from paper_1208_0302_b200 import workloads as W  # noqa: E402
 # kernel changes (r1a: 477, r1b: 280, r1c: 265.7, r1f: 263.3), so `frac` is the FP32-pipe utilisation, not an inflated textbook
 # count.  See DESIGN.md "Measurement".  config0 (one line) is not the bench default and carries an estimate.
 FLOP_PER_POINT = {"config0_tiny": 150.0, "config1_map256": 263.3, "config3_fulldisc": 263.3, "config4_stress11": 264.0}
+# MUFU (SFU / XU pipe) instructions per wavelength point, same capture: 6 Voigt reciprocals + 1 for the determinant (+ 1 for the
+# field-free profile of the 11-parameter model)
+MUFU_PER_POINT = 7.13
 # DRAM traffic of ga_invert_kernel per pixel, from the same capture (dram__bytes_read.sum + write.sum) / pixels
 DRAM_BYTES_PER_PIXEL_NCU = 8.496128e6 / 4096      # at L = 128 (2088 algorithmic bytes); scaled by 16 L + 40 for other grids
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
@@ -381,6 +384,9 @@ def run_b200(args):
                          "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt,
                          "peak_measured_ffma_tflops": probe["ffma"]["tflops"],
                          "mufu_per_s_measured": probe["mufu"]["thread_inst_per_s"],
+                         "sfu": {"mufu_per_lambda_point": MUFU_PER_POINT, "achieved_per_s": MUFU_PER_POINT * points_per_launch / launch_s,
+                                 "peak_per_s_measured": probe["mufu"]["thread_inst_per_s"],
+                                 "frac": MUFU_PER_POINT * points_per_launch / launch_s / probe["mufu"]["thread_inst_per_s"]},
                          "peak_basis": "148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (max SM clock)" % sm_max,
                          "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / sm_max)) if clocks.get("sm_mhz") else None},
             "clocks": clocks, "gpu_launches": args.steps, "e2e": e2e}
