@@ -239,7 +239,7 @@ def build_inputs(cfg, n_pixels, side, rank, torch, B):
     return ld, obs, mask_t, mu_t, n_active, truth
 
 
-def bench_me_synth(torch, B, peaks, P=1_000_000):
+def bench_me_synth(torch, B, peaks, P=1_000_000, chi2_only=True):
     """BASELINE config 2: forward synthesis of P prior draws on the two-line 128-point grid, IQUV output + chi2 against
     one fixed profile (and chi2 only, to separate ALU from the store stream).  Not the headline metric: reported beside it."""
     c2 = W.config2(P)
@@ -252,7 +252,10 @@ def bench_me_synth(torch, B, peaks, P=1_000_000):
     out = torch.empty((P, 4, L), dtype=torch.float32, device="cuda")
     chi = torch.empty((P,), dtype=torch.float32, device="cuda")
     res = {}
-    for name, kw in (("stokes_and_chi2", dict(out_stokes=out, out_chi2=chi)), ("chi2_only", dict(out_chi2=chi, want_stokes=False))):
+    legs = [("stokes_and_chi2", dict(out_stokes=out, out_chi2=chi))]
+    if chi2_only:
+        legs.append(("chi2_only", dict(out_chi2=chi, want_stokes=False)))
+    for name, kw in legs:
         for _ in range(3):
             B.me_synth(params, lam, ld, obs_ref=obs_ref, w_over_sigma=wos, **kw)
         torch.cuda.synchronize()
@@ -392,6 +395,11 @@ def run_b200(args):
             "clocks": clocks, "gpu_launches": args.steps, "e2e": e2e}
     if not args.no_aux:
         line["me_synth_config2"] = bench_me_synth(torch, B, peaks)
+        # BASELINE config 2's saturation trace: P = 1e4 .. 1e7 with the full [P,4,L] output (20.5 GB at 1e7)
+        line["me_synth_config2"]["saturation"] = {
+            str(P): round(bench_me_synth(torch, B, peaks, P=P, chi2_only=False)["stokes_and_chi2"]["syntheses_per_s"])
+            for P in (10_000, 100_000, 10_000_000)}
+        torch.cuda.empty_cache()
     if not args.no_cpu_baseline:
         from oracle import api as orc
         cores = orc.hardware_threads()
