@@ -173,8 +173,9 @@ MEDEV void faddeeva_far_acc(f2 v, f2 r2, const FarCoef& c, f2& sr, f2& si) {
 MEDEV FarCoef far_load(const float4* p, int stride) {
     float4 x, y;
     const unsigned ax = (unsigned)__cvta_generic_to_shared(p), ay = (unsigned)__cvta_generic_to_shared(p + stride);
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(ax));
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(y.x), "=f"(y.y), "=f"(y.z), "=f"(y.w) : "r"(ay));
+    // "memory": the compiler must not sink or drop far_store's plain stores, which only these loads read
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(ax) : "memory");
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(y.x), "=f"(y.y), "=f"(y.z), "=f"(y.w) : "r"(ay) : "memory");
     FarCoef c;
     c.x3 = x.x; c.x2 = x.y; c.x1 = x.z; c.x0 = x.w; c.y3 = y.x; c.y2 = y.y; c.y1 = y.z; c.y0 = y.w;
     return c;
