@@ -140,6 +140,16 @@ def uncertainty_from_chi2(chi2v, M, h, active=None):
     return out
 
 
+def seeds(obs, lam, lines, cfg):
+    """Reading S1: obs[N,4,L] -> [N,3] = centre-of-gravity B_los [G], and the 10-bit box coordinates (q_B, q_gamma) of the seed."""
+    obs, lam = _f64(obs), _f64(lam)
+    N, L = obs.shape[0], lam.size
+    out = np.empty((N, 3))
+    lib().orc_seeds(_p(obs, C.c_double), C.c_int64(N), _p(lam, C.c_double), C.c_int(L), *lines.args(),
+                    C.c_double(cfg["lo"][0]), C.c_double(cfg["hi"][0]), C.c_int(int(cfg["log_scale"][0])), _p(out, C.c_double))
+    return out
+
+
 def sobol(n0, count, dims):
     out = np.zeros((count, dims), dtype=np.uint32)
     lib().orc_sobol(C.c_uint32(n0), C.c_int(count), C.c_int(dims), _p(out, C.c_uint32))

@@ -130,6 +130,16 @@ void orc_uncertainty_from_chi2(const double* chi2v, int M, double h, const int* 
     uncertainty_from_chi2(chi2v, M, h, active, sigma_u);
 }
 
+// Heuristic seeds of one batch: obs[N][4][L] -> out[N][3] = B_los [G], q_B, q_gamma (reading S1).
+void orc_seeds(const double* obs, int64_t N, const double* lambda, int L,
+               int n_lines, const double* lambda0, const double* strength, const int* n_comp,
+               const double* shift, const double* weight, const int* kind, double lambda_ref,
+               double b_lo, double b_hi, int b_log, double* out) {
+    Lines ln = make_lines(n_lines, lambda0, strength, n_comp, shift, weight, kind, lambda_ref);
+    GaCfg c; c.lo[P_B] = b_lo; c.hi[P_B] = b_hi; c.log_scale[P_B] = b_log;
+    for (int64_t n = 0; n < N; ++n) pixel_seeds(obs + n * 4 * L, lambda, L, ln, c, out + n * 3);
+}
+
 // count Sobol' points starting at index n0, dims dimensions: out[count][dims] (32-bit fixed point).
 void orc_sobol(uint32_t n0, int count, int dims, uint32_t* out) {
     for (int i = 0; i < count; ++i)

@@ -215,6 +215,53 @@ void pixel_prologue(const double* obs, int L, const GaCfg& c, double out[6]) {
     }
 }
 
+// S1: "the initial population includes ... the longitudinal field strength estimated from the
+// center-of-gravity approach by Rees & Semel (1979) ... [and] the trivial non-magnetic solution".  The paper prints no
+// formula; the textbook centre-of-gravity method is taken:
+//   lambda_+- = sum_j lambda_j (I_c - (I_j +- V_j)) / sum_j (I_c - (I_j +- V_j)),   B_los = (lambda_+ - lambda_-) / (2 C g lambda_0^2),
+// C = 4.66857e-13 /A/G, on the line with the largest g lambda_0^2 (g = centre of gravity of its sigma_red shifts), over
+// the samples closer to that line than half the distance to the nearest other line (all samples for a single line), with
+// I_c the largest observed intensity.  With reading F4 a positive blue V lobe deepens I - V on the blue side, so
+// lambda_+ > lambda_- and B_los > 0 means gamma < 90 deg.  Seeded members (generation 0 only, pop >= 3):
+//   slot P-1: B gene = 0 (the non-magnetic solution); slot P-2: B = |B_los| clamped to its box, gamma at the end of its
+//   (polarity-cut) box that matches the sign of B_los; both box coordinates quantised to 10 bits (a heuristic needs no
+//   more, and the two implementations then agree on the gene except at a rounding boundary); other genes as drawn.
+void pixel_seeds(const double* obs, const double* lambda, int L, const Lines& ln, const GaCfg& c, double out[3]) {
+    const double CZ = 4.66857e-13;
+    int best = 0; double gbest = -1.0, sens = -1.0;
+    for (size_t l = 0; l < ln.lines.size(); ++l) {
+        double g = 0.0;
+        for (const Component& k : ln.lines[l].comps) if (k.kind == 1) g += k.weight * k.shift;
+        const double s = g * ln.lines[l].lambda0 * ln.lines[l].lambda0;
+        if (s > sens) { sens = s; best = (int)l; gbest = g; }
+    }
+    const double l0 = ln.lines[best].lambda0;
+    double hw = std::numeric_limits<double>::infinity();
+    for (size_t l = 0; l < ln.lines.size(); ++l)
+        if ((int)l != best) hw = std::fmin(hw, 0.5 * std::fabs(ln.lines[l].lambda0 - l0));
+    double ic = obs[0];
+    for (int j = 1; j < L; ++j) ic = std::fmax(ic, obs[j]);
+    double sp = 0, sm = 0, lp = 0, lm = 0;
+    for (int j = 0; j < L; ++j) {
+        const double d = lambda[j] - l0;
+        if (std::fabs(d) > hw) continue;
+        const double ap = ic - (obs[j] + obs[3 * L + j]), am = ic - (obs[j] - obs[3 * L + j]);
+        sp += ap; sm += am; lp += d * ap; lm += d * am;
+    }
+    double blos = 0.0;
+    if (sp > 0.0 && sm > 0.0 && gbest > 0.0) blos = (lp / sp - lm / sm) / (2.0 * CZ * gbest * l0 * l0);
+    const double b = std::fmin(std::fmax(std::fabs(blos), c.lo[P_B]), c.hi[P_B]);
+    double u = 0.0;
+    if (c.hi[P_B] > c.lo[P_B]) u = c.log_scale[P_B] ? std::log(b / c.lo[P_B]) / std::log(c.hi[P_B] / c.lo[P_B]) : (b - c.lo[P_B]) / (c.hi[P_B] - c.lo[P_B]);
+    out[0] = blos;
+    out[1] = std::rint(u * 1023.0);
+    out[2] = blos >= 0.0 ? 0.0 : 1023.0;
+}
+
+// stored gene for a 10-bit box coordinate q: the real-coded variant holds q / 1023 (one binary32 division), the
+// binary-coded variant the 16-bit code q << 6
+static float seed_gene(double q, const GaCfg& c) { return c.variant == 1 ? (float)(64.0 * q) : (float)q / 1023.0f; }
+
 void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c0,
                      uint64_t pixel, double* best_params, double* best_chi2, float* best_genes, double* trace) {
     GaCfg c = c0;                                                  // per-pixel weights and inclination box
@@ -228,6 +275,13 @@ void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, 
     std::vector<float> genes(c.pop * M), next(c.pop * M);
     std::vector<double> f(c.pop), fnext(c.pop), model(4 * L);
     ga_init(pixel, c, genes.data());
+    if ((c0.prologue & 4) && c.pop >= 3) {                          // reading S1
+        double sd[3];
+        pixel_seeds(obs, lambda, L, ln, c, sd);
+        genes[(c.pop - 1) * M + P_B] = seed_gene(0.0, c);
+        genes[(c.pop - 2) * M + P_B] = seed_gene(sd[1], c);
+        genes[(c.pop - 2) * M + P_GAMMA] = seed_gene(sd[2], c);
+    }
     for (int i = 0; i < c.pop; ++i) f[i] = fitness(&genes[i * M], obs, mu, lambda, L, ln, c, model);
     if (trace) trace[0] = f[argmin(f.data(), c.pop)];
     for (int t = 1; t <= c.generations; ++t) {

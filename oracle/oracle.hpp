@@ -92,12 +92,17 @@ struct GaCfg {
     int log_scale[MAXPAR], periodic[MAXPAR];
     double w[4], sigma[4];
     uint64_t seed;
-    int prologue = 0;                          // bit 0: inverse-max weights (eq. 20-23), bit 1: polarity restriction of gamma
+    int prologue = 0;                          // bit 0: inverse-max weights (eq. 20-23), bit 1: polarity restriction of gamma,
+                                               // bit 2: heuristic seeds in P0 (reading S1)
 };
 // Per-pixel prologue of the paper (SURVEY.md par. 8(f)-3; readings W1, P1 of DESIGN.md), computed from the observed
 // profile alone.  out[6] = w_I, w_Q, w_U, w_V (eq. 20-23; unchanged c.w if bit 0 is clear) and the
 // inclination box [gamma_lo, gamma_hi] (the configured box if bit 1 is clear).
 void pixel_prologue(const double* obs, int L, const GaCfg& c, double out[6]);
+// Heuristic seeds (reading S1 of DESIGN.md): the centre-of-gravity longitudinal field B_los (Rees &
+// Semel 1979) of the most Zeeman-sensitive line, in Gauss (signed), and the box coordinates (u_B, u_gamma) of the seeded
+// member, quantised to 10 bits: out[3] = B_los, q_B, q_gamma (q in 0..1023).
+void pixel_seeds(const double* obs, const double* lambda, int L, const Lines& ln, const GaCfg& c, double out[3]);
 double decode_gene(float g, double lo, double hi, int log_scale);
 float gene_value(float stored, const GaCfg& c);   // variant 1: 16-bit code -> g = k / 65535 (eq. 5), rounded to binary32
 // Next generation from (genes[pop][NPAR], chi2[pop]) at generation t >= 1 for global pixel id `pixel`.
