@@ -113,6 +113,10 @@ typedef struct {
                                     stokes_weight;
                                  2: the inclination box [lo[1], hi[1]] is cut to the polarity given by the order of the
                                     Stokes-V lobes: positive lobe on the blue side => gamma <= 90 deg.
+                                 4: two heuristic members replace the last two slots of the initial population
+                                    (reading S1): B = |B_los| from the centre of gravity of I +- V
+                                    (Rees & Semel 1979) with gamma at the matching end of its box, and the non-magnetic
+                                    solution B = lo[0]; other genes as drawn. Needs pop >= 3.
                                  ga_fitness ignores these flags (fixed weights, configured box). */
 } ga_cfg;
 
@@ -145,9 +149,10 @@ int ga_step(const float* genes_in /*[N,pop,n_params]*/, const float* chi2_in /*[
 int ga_fitness(const float* genes /*[N,pop,n_params]*/, const float* obs /*[N,4,L]*/, int64_t N, const float* sigma /*host[4]*/,
                const double* lambda_grid_A, int L, const me_line_data* line_data, const ga_cfg* cfg,
                float* chi2_out /*[N,pop]*/, void* stream);
-/* The per-pixel prologue alone: out device [N,6] f32 = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them. */
-int ga_prologue(const float* obs /*[N,4,L]*/, int64_t N, int L, const float* sigma /*host[4]*/, const ga_cfg* cfg,
-                float* out, void* stream);
+/* The per-pixel prologue alone: out device [N,9] f32 = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them,
+ * then B_los [G] and the stored genes (B, gamma) of the centre-of-gravity member (0 unless prologue bit 4). */
+int ga_prologue(const float* obs /*[N,4,L]*/, int64_t N, const float* sigma /*host[4]*/, const double* lambda_grid_A, int L,
+                const me_line_data* line_data, const ga_cfg* cfg, float* out, void* stream);
 /* Generation-0 population (reading G2): genes_out device [N,pop,n_params]. */
 int ga_init(int64_t N, const ga_cfg* cfg, int n_params, uint64_t seed, float* genes_out, void* stream);
 /* One Philox4x32-10 block computed ON THE DEVICE; out is a HOST pointer; synchronises. */

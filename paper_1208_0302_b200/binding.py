@@ -267,15 +267,17 @@ def me_peak_probe(kind, iters, blocks, scratch):
     return blocks * 256 * iters * 32
 
 
-def ga_prologue(obs, cfg):
-    """obs: CUDA f32 [N,4,L]. Returns [N,6]: w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them (cfg["prologue"])."""
+def ga_prologue(obs, lam, line_data, cfg):
+    """obs: CUDA f32 [N,4,L]. Returns [N,9]: w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them, then B_los [G] and
+    the stored genes (B, gamma) of the centre-of-gravity member (cfg["prologue"] bit flags)."""
     import torch
-    N, L = obs.shape[0], obs.shape[2]
+    N = obs.shape[0]
+    lam, lam_p, L = _grid(lam)
     c, keep = make_ga_cfg(cfg)
     sig = np.ascontiguousarray(cfg["sigma"], dtype=np.float32)
-    out = torch.empty((N, 6), dtype=torch.float32, device=obs.device)
-    _check(lib().ga_prologue(_dev(obs, torch.float32, "obs"), C.c_int64(N), C.c_int(L), sig.ctypes.data_as(C.POINTER(C.c_float)),
-                             C.byref(c), _dev(out, torch.float32, "out"), _stream()), "ga_prologue")
+    out = torch.empty((N, 9), dtype=torch.float32, device=obs.device)
+    _check(lib().ga_prologue(_dev(obs, torch.float32, "obs"), C.c_int64(N), sig.ctypes.data_as(C.POINTER(C.c_float)), lam_p, L,
+                             C.byref(line_data.c), C.byref(c), _dev(out, torch.float32, "out"), _stream()), "ga_prologue")
     return out
 
 

@@ -97,7 +97,7 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
     if (c->tournament_k < 1 || c->tournament_k > 4) return ME_ERR_RANGE;
     if (c->elite != 1) return ME_ERR_UNSUPPORTED;
     if (c->variant != 0 && c->variant != 1) return ME_ERR_RANGE;
-    if (c->prologue < 0 || c->prologue > 3) return ME_ERR_RANGE;
+    if (c->prologue < 0 || c->prologue > 7) return ME_ERR_RANGE;
     if ((c->prologue & 2) && c->log_scale[1]) return ME_ERR_UNSUPPORTED;      // the polarity box is linear in gamma
     if (!(c->p_cross >= 0.f && c->p_cross <= 1.f) || !(c->p_mut >= 0.f && c->p_mut <= 1.f)) return ME_ERR_RANGE;
     if (c->pixel_id_base < 0 || N < 0 || (uint64_t)c->pixel_id_base + (uint64_t)N > 0x100000000ULL) return ME_ERR_RANGE;
@@ -140,6 +140,26 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
             g.mut_scale[t] = (float)((double)c->mut_scale0 * std::pow((double)c->mut_scale_end / (double)c->mut_scale0, (double)t / G));
     }
     return ME_OK;
+}
+
+// Reading S1: the line the centre-of-gravity seed is taken on (largest g lambda^2, g = centre of gravity of the sigma_red
+// shifts), its window half-width and the wavelength-to-field scale 1 / (2 C g lambda^2).
+void fill_seed_desc(const me_line_data* ld, me::GaDesc& g) {
+    g.seed_line = 0; g.seed_hw = INFINITY; g.seed_scale = 0.0f;
+    double best = -1.0, gbest = 0.0;
+    for (int l = 0; l < ld->n_lines; ++l) {
+        const me_line& ln = ld->lines[l];
+        double geff = 0.0;
+        for (int c = 0; c < ln.n_comp; ++c) if (ln.kind[c] == 1) geff += (double)ln.weight[c] * (double)ln.shift[c];
+        const double s = geff * ln.lambda0_A * ln.lambda0_A;
+        if (s > best) { best = s; g.seed_line = l; gbest = geff; }
+    }
+    const double l0 = ld->lines[g.seed_line].lambda0_A;
+    double hw = INFINITY;
+    for (int l = 0; l < ld->n_lines; ++l)
+        if (l != g.seed_line) hw = std::fmin(hw, 0.5 * std::fabs(ld->lines[l].lambda0_A - l0));
+    g.seed_hw = (float)hw;
+    if (gbest > 0.0) g.seed_scale = (float)(1.0 / (2.0 * ZEEMAN * gbest * l0 * l0));
 }
 
 }  // namespace
@@ -192,6 +212,7 @@ int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sig
     if (rc != ME_OK) return rc;
     rc = build_ga_desc(cfg, sd.npar, sigma, L, seed, N, true, gd);
     if (rc != ME_OK) return rc;
+    fill_seed_desc(line_data, gd);
     if (N == 0) return ME_OK;
     if (obs == nullptr || out_params == nullptr || out_chi2 == nullptr) return ME_ERR_NULL;
     cudaError_t e = me::launch_ga_invert(sd, gd, obs, mask, cfg->mu, N, out_params, out_chi2, (cudaStream_t)stream);
@@ -237,14 +258,17 @@ int ga_step(const float* genes_in, const float* chi2_in, int64_t N, int generati
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 
-int ga_prologue(const float* obs, int64_t N, int L, const float* sigma, const ga_cfg* cfg, float* out, void* stream) {
-    if (L < 2 || L > ME_MAX_L) return ME_ERR_SHAPE;
-    me::GaDesc gd;
-    int rc = build_ga_desc(cfg, ME_NPAR, sigma, L, 0, N, true, gd);
+int ga_prologue(const float* obs, int64_t N, const float* sigma, const double* lambda_grid_A, int L,
+                const me_line_data* line_data, const ga_cfg* cfg, float* out, void* stream) {
+    me::SynthDesc sd; me::GaDesc gd;
+    int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
     if (rc != ME_OK) return rc;
+    rc = build_ga_desc(cfg, sd.npar, sigma, L, 0, N, true, gd);
+    if (rc != ME_OK) return rc;
+    fill_seed_desc(line_data, gd);
     if (N == 0) return ME_OK;
     if (obs == nullptr || out == nullptr) return ME_ERR_NULL;
-    cudaError_t e = me::launch_ga_prologue(gd, obs, N, L, out, (cudaStream_t)stream);
+    cudaError_t e = me::launch_ga_prologue(&sd, gd, obs, N, L, out, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 

@@ -52,8 +52,11 @@ struct GaDesc {
     float lo[ME_MAX_NPAR], span[ME_MAX_NPAR], log2ratio[ME_MAX_NPAR];
     int log_scale[ME_MAX_NPAR], periodic[ME_MAX_NPAR];
     float mut_scale[ME_MAX_GEN + 1];    // s_t, t = 0..generations
-    // per-pixel prologue (readings W1, P1): bit 0 inverse-max weights, bit 1 polarity restriction
+    // per-pixel prologue (readings W1, P1, S1): bit 0 inverse-max weights, bit 1 polarity restriction, bit 2 seeds
     int prologue;
+    int seed_line;                      // S1: the line with the largest g lambda^2
+    float seed_hw;                      // half-width of its window (half the distance to the nearest other line, or +Inf)
+    float seed_scale;                   // 1 / (2 C g lambda^2)   [G per A]
     float w_cfg[4], sigma[4];           // configured w_s and sigma_s (w2 above is (w_s / sigma_s)^2)
     // variant 1 (the paper's binary-coded GA, readings V0-V5 of DESIGN.md)
     int variant;                        // 0 real-coded operators, 1 binary-coded
@@ -588,9 +591,11 @@ __device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int 
 
 // Per-pixel prologue (readings W1, P1; eq. 20-23, polarity PAPER.md:278), run by ONE warp on the staged
 // observation (pair-interleaved layout of stage_obs).  pix[0..3] = (w_s / sigma_s)^2, pix[4] = gamma_lo, pix[5] = gamma
-// span, pix[6] = gamma_hi; without flags these are the configured values.
-#define ME_PIX_WORDS 8
-__device__ __forceinline__ void pixel_prologue(const float* obs_s, int L, const GaDesc& gd, float* pix, bool writer) {
+// span, pix[6] = gamma_hi; without flags these are the configured values.  Bit 2 (reading S1): pix[7],
+// pix[8] = stored genes (B, gamma) of the centre-of-gravity member, pix[9] = B_los [G]; `off` = sd.off[gd.seed_line].
+#define ME_PIX_WORDS 12
+__device__ __forceinline__ void pixel_prologue(const float* obs_s, int L, const GaDesc& gd, float* pix, bool writer,
+                                               const float* off = nullptr) {
     const int lane = threadIdx.x & 31;
     const float INF = __int_as_float(0x7f800000);
     float imax = -INF, imin = INF, mq = 0.f, mu_ = 0.f, mv = 0.f, vmax = -INF, vmin = INF;
@@ -632,6 +637,35 @@ __device__ __forceinline__ void pixel_prologue(const float* obs_s, int L, const 
             else glo = fmaxf(glo, 90.0f);
         }
         pix[4] = glo; pix[5] = (gd.prologue & 2) ? ghi - glo : gd.span[1]; pix[6] = ghi;
+    }
+    if ((gd.prologue & 4) && off != nullptr) {               // S1: centre of gravity of I +- V (Rees & Semel 1979)
+        float sp = 0.f, sm = 0.f, lp = 0.f, lm = 0.f;
+#pragma unroll 1
+        for (int j = lane; j < L; j += 32) {
+            const float dl = off[j];
+            if (fabsf(dl) > gd.seed_hw) continue;
+            const float* o = obs_s + 8 * (j >> 1) + (j & 1);
+            const float ap = imax - (o[0] + o[6]), am = imax - (o[0] - o[6]);
+            sp += ap; sm += am; lp = fmaf(dl, ap, lp); lm = fmaf(dl, am, lm);
+        }
+#pragma unroll 1
+        for (int s = 16; s > 0; s >>= 1) {
+            sp += __shfl_xor_sync(0xffffffffu, sp, s); sm += __shfl_xor_sync(0xffffffffu, sm, s);
+            lp += __shfl_xor_sync(0xffffffffu, lp, s); lm += __shfl_xor_sync(0xffffffffu, lm, s);
+        }
+        if (writer) {
+            float blos = 0.f;
+            if (sp > 0.f && sm > 0.f) blos = (lp / sp - lm / sm) * gd.seed_scale;
+            const float hiB = gd.log_scale[0] ? gd.lo[0] * exp2f(gd.log2ratio[0]) : gd.lo[0] + gd.span[0];
+            const float b = fminf(fmaxf(fabsf(blos), gd.lo[0]), hiB);
+            float u = 0.f;
+            if (gd.log_scale[0]) { if (gd.log2ratio[0] != 0.f) u = log2f(b / gd.lo[0]) / gd.log2ratio[0]; }
+            else if (gd.span[0] != 0.f) u = (b - gd.lo[0]) / gd.span[0];
+            const float qb = rintf(u * 1023.0f), qg = blos >= 0.f ? 0.f : 1023.0f;
+            pix[7] = gd.variant ? 64.0f * qb : __fdiv_rn(qb, 1023.0f);
+            pix[8] = gd.variant ? 64.0f * qg : __fdiv_rn(qg, 1023.0f);
+            pix[9] = blos;
+        }
     }
 }
 

@@ -116,7 +116,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         __syncthreads();                                   // previous pixel's shared memory is no longer read
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
         __syncthreads();
-        pixel_prologue(obs_s, L, gd, pix_s, tid == 0);      // every warp reduces, thread 0 writes; visible after the next barrier
+        pixel_prologue(obs_s, L, gd, pix_s, tid == 0, sd.off[gd.seed_line]);   // every warp reduces, thread 0 writes; visible after the next barrier
 
         // generations 0..G with ONE fitness call site (keeps the loop body inside the instruction cache)
         float g[M];
@@ -141,6 +141,10 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
                 if (t == 0) {
                     if (gd.variant) sobol_genes<M>(g, pixel, (uint32_t)tid + 1u, gd);  // reading V1
                     else init_genes<M>(g, pixel, (uint32_t)tid, gd);                  // reading G2
+                    if ((gd.prologue & 4) && pop >= 3) {                              // reading S1: heuristic members of P0
+                        if (tid == pop - 1) g[0] = 0.0f;                              // the non-magnetic solution
+                        if (tid == pop - 2) { g[0] = pix_s[7]; g[1] = pix_s[8]; }     // centre-of-gravity longitudinal field
+                    }
                 } else if (tid == 0) {
 #pragma unroll
                     for (int j = 0; j < M; ++j) g[j] = gprev[ie * M + j];

@@ -76,9 +76,10 @@ __global__ void ga_init_kernel(const __grid_constant__ GaDesc gd, int64_t N, flo
     for (int j = 0; j < M; ++j) genes_out[k * M + j] = g[j];
 }
 
-// The per-pixel prologue alone (one warp per pixel): out[n][6] = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi.
+// The per-pixel prologue alone (one warp per pixel): out[n][9] = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi, B_los, and the
+// stored genes (B, gamma) of the centre-of-gravity member.  off: device copy of lambda_j - lambda_(seed line), or nullptr.
 __global__ void ga_prologue_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ obs, int64_t N, int L,
-                                   float* __restrict__ out) {
+                                   const float* __restrict__ off, float* __restrict__ out) {
     extern __shared__ float4 smem4[];
     float* obs_s = reinterpret_cast<float*>(smem4);
     float* pix_s = obs_s + 8 * ((L + 1) >> 1);
@@ -86,10 +87,15 @@ __global__ void ga_prologue_kernel(const __grid_constant__ GaDesc gd, const floa
         __syncwarp();
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, threadIdx.x, 32);
         __syncwarp();
-        pixel_prologue(obs_s, L, gd, pix_s, threadIdx.x == 0);
+        if (threadIdx.x == 0) pix_s[7] = pix_s[8] = pix_s[9] = 0.f;
         __syncwarp();
-        if (threadIdx.x < 4) out[n * 6 + threadIdx.x] = sqrtf(pix_s[threadIdx.x]) * gd.sigma[threadIdx.x];   // back to w_s
-        if (threadIdx.x == 4) { out[n * 6 + 4] = pix_s[4]; out[n * 6 + 5] = pix_s[6]; }
+        pixel_prologue(obs_s, L, gd, pix_s, threadIdx.x == 0, off);
+        __syncwarp();
+        if (threadIdx.x < 4) out[n * 9 + threadIdx.x] = sqrtf(pix_s[threadIdx.x]) * gd.sigma[threadIdx.x];   // back to w_s
+        if (threadIdx.x == 4) {
+            out[n * 9 + 4] = pix_s[4]; out[n * 9 + 5] = pix_s[6];
+            out[n * 9 + 6] = pix_s[9]; out[n * 9 + 7] = pix_s[7]; out[n * 9 + 8] = pix_s[8];
+        }
     }
 }
 
@@ -179,10 +185,20 @@ cudaError_t launch_ga_init(const GaDesc& gd, int npar, int64_t N, float* genes_o
     return cudaGetLastError();
 }
 
-cudaError_t launch_ga_prologue(const GaDesc& gd, const float* obs, int64_t N, int L, float* out, cudaStream_t st) {
+cudaError_t launch_ga_prologue(const SynthDesc* sd, const GaDesc& gd, const float* obs, int64_t N, int L, float* out,
+                               cudaStream_t st) {
     const size_t smem = (size_t)32 * ((L + 1) / 2) + ME_PIX_WORDS * 4;
-    ga_prologue_kernel<<<grid_for(N), 32, smem, st>>>(gd, obs, N, L, out);
-    return cudaGetLastError();
+    float* off = nullptr;                                    // hook only: a stream-ordered scratch copy of the offsets
+    if (sd != nullptr && (gd.prologue & 4)) {
+        cudaError_t e = cudaMallocAsync(&off, (size_t)L * 4, st);
+        if (e != cudaSuccess) return e;
+        e = cudaMemcpyAsync(off, sd->off[gd.seed_line], (size_t)L * 4, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return e;
+    }
+    ga_prologue_kernel<<<grid_for(N), 32, smem, st>>>(gd, obs, N, L, off, out);
+    cudaError_t e = cudaGetLastError();
+    if (off != nullptr) { cudaStreamSynchronize(st); cudaFreeAsync(off, st); }   // the host copy source is the caller's stack
+    return e;
 }
 
 cudaError_t launch_philox(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3, int64_t n,

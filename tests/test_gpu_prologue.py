@@ -36,12 +36,59 @@ def test_prologue_hook_vs_oracle(B, which, flags):
     obs[6, 3] = 0.0                                            # no V signal at all: argmax = argmin = 0 -> [90, 180]
     cfg = dict(c["ga"], prologue=flags)
     want = orc.prologue(obs, cfg)
-    got = B.ga_prologue(dev(obs), cfg).cpu().numpy().astype(np.float64)
-    assert np.array_equal(got[:, 4:], want[:, 4:])            # the polarity box is an exact decision
+    ld = B.line_data_from_workload(c["lines"], True)
+    got = B.ga_prologue(dev(obs), c["lam"], ld, cfg).cpu().numpy().astype(np.float64)
+    assert np.array_equal(got[:, 4:6], want[:, 4:])           # the polarity box is an exact decision
+    assert np.all(got[:, 6:] == 0.0)                          # no seeds asked for
     assert np.max(np.abs(got[:, :4] - want[:, :4]) / want[:, :4]) < 1e-6
     if flags & 2:
         strong = truth[:, 0] > 800.0                           # strong fields: the lobe order gives the true polarity
         assert np.mean((want[strong, 5] <= 90.0) == (truth[strong, 1] < 90.0)) > 0.97
+
+
+@pytest.mark.parametrize("which,variant", [("config0", 0), ("config1", 0), ("config1", 1)])
+def test_seeds_hook_vs_oracle(B, which, variant):
+    c = W.config0() if which == "config0" else W.config1()
+    N = 400
+    truth, obs, ln = make_obs(c, N, threads=NTHREADS)
+    cfg = dict(c["ga"], prologue=4, variant=variant)
+    want = orc.seeds(obs, c["lam"], ln, cfg)
+    ld = B.line_data_from_workload(c["lines"], True)
+    got = B.ga_prologue(dev(obs), c["lam"], ld, cfg).cpu().numpy().astype(np.float64)
+    big = np.abs(want[:, 0]) > 5.0
+    assert np.max(np.abs(got[big, 6] - want[big, 0]) / np.abs(want[big, 0])) < 2e-3     # B_los: FP32 centroid differences
+    assert np.max(np.abs(got[:, 6] - want[:, 0])) < 0.05                                 # ... a few hundredths of a Gauss
+    gene = (lambda q: 64.0 * q) if variant else (lambda q: (q.astype(np.float32) / np.float32(1023.0)).astype(np.float64))
+    same_b = got[:, 7] == gene(want[:, 1])
+    same_g = got[:, 8] == gene(want[:, 2])
+    assert same_b.mean() > 0.97 and same_g.mean() > 0.97      # 10-bit quantisation: equal except at a rounding boundary / B_los ~ 0
+    off = np.abs(got[~same_b, 7] - gene(want[~same_b, 1]))
+    assert off.size == 0 or off.max() <= (64.0 if variant else 1.01 / 1023.0)           # and then by one step only
+
+
+def test_inversion_with_seeds_parity(B):
+    c0 = W.config0()
+    N = 64
+    truth, obs, ln = make_obs(c0, N, threads=NTHREADS)
+    ld = B.line_data_from_workload(c0["lines"], True)
+    for variant in (0, 1):
+        ga = dict(c0["ga"], prologue=7, variant=variant)
+        res = orc.ga_invert(obs, c0["lam"], ln, ga, seed=W.SEED_GA, threads=NTHREADS)
+        gp, gc = B.ga_invert(dev(obs), c0["lam"], ld, ga, W.SEED_GA)
+        gc = gc.cpu().numpy().astype(np.float64)
+        same = np.abs(gc - res["chi2"]) <= 2e-4 * res["chi2"]
+        assert same.mean() >= 0.85, (variant, same.mean())
+        assert abs(np.median(gc) - np.median(res["chi2"])) <= 0.01 * np.median(res["chi2"])
+    # zero generations, everything but (B, gamma) fixed at the truth: the centre-of-gravity member wins on both sides
+    strong = np.flatnonzero((truth[:, 0] > 800.0) & (np.abs(np.cos(np.radians(truth[:, 1]))) > 0.8))[:6]
+    for n in strong:
+        ga = W.ga_config(32, 0, prologue=4)
+        for j in range(2, 9):
+            ga["lo"][j] = ga["hi"][j] = truth[n, j]
+        r = orc.ga_invert(obs[n:n + 1], c0["lam"], ln, ga, seed=2, pixel_base=int(n))
+        p, c = B.ga_invert(dev(obs[n:n + 1]), c0["lam"], ld, ga, 2, pixel_id_base=int(n))
+        assert abs(float(c[0]) - r["chi2"][0]) <= 2e-4 * r["chi2"][0]
+        assert np.allclose(p.cpu().numpy()[0], r["params"][0], rtol=2e-3, atol=1e-3)
 
 
 def test_inversion_with_prologue_parity(B):
