@@ -145,27 +145,26 @@ MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
 // With v^2 = 1/r - a^2,  Re/Im of i s (C0 + C1 q + C2 q^2) become
 //   H = a r X(r),  X = C0 + 3 C1 r + (5 C2 - 4 a^2 C1) r^2 - 20 a^2 C2 r^3 + 16 a^4 C2 r^4
 //   F = v r Y(r),  Y = C0 +   C1 r + (  C2 - 4 a^2 C1) r^2 - 12 a^2 C2 r^3 + 16 a^4 C2 r^4
-// (the r^4 terms are < 1e-8 relative for a <= FAD_FAR_AMAX and are dropped).  The coefficients depend on the individual
+// (the r^4 terms are < 1e-8 relative for a <= FAD_FAR_AMAX; the r^3 terms are < 3e-6 relative = 1e-8 absolute in H and
+// 5e-8 in F, below the FP32 rounding of the evaluation itself: both are dropped, X and Y are evaluated as quadratics).  The coefficients depend on the individual
 // only, so each Horner step is FFMA2 (pair x pair + scalar) -- the full-rate operand form (profiles/r1c peaks: an
 // FFMA2 whose ADDEND is a register pair runs at 0.77 of that rate) -- and the line strength r_l and the factor a are
-// folded into them:  fx = a r_l (x3, x2, x1, C0),  fy = r_l (y3, y2, y1, C0).
-struct FarCoef { float x3, x2, x1, x0, y3, y2, y1, y0; };
+// folded into them:  fx = a r_l (x2, x1, C0),  fy = r_l (y2, y1, C0).
+struct FarCoef { float x2, x1, x0, y2, y1, y0; };
 
 MEDEV FarCoef far_coef(float a, float strength) {
     FarCoef c;
     const float a2 = a * a, sa = strength * a;
     c.x0 = sa * FAD_C0; c.x1 = sa * (3.0f * FAD_C1); c.x2 = sa * fmaf(-4.0f * FAD_C1, a2, 5.0f * FAD_C2);
-    c.x3 = sa * (-20.0f * FAD_C2) * a2;
     c.y0 = strength * FAD_C0; c.y1 = strength * FAD_C1; c.y2 = strength * fmaf(-4.0f * FAD_C1, a2, FAD_C2);
-    c.y3 = strength * (-12.0f * FAD_C2) * a2;
     return c;
 }
 
 // accumulates r_l w(v + i a) into (sr, si)
 MEDEV void faddeeva_far_acc(f2 v, f2 r2, const FarCoef& c, f2& sr, f2& si) {
     const f2 r = rcp2(r2);
-    const f2 X = fma2(fma2(fma2(bc(c.x3), r, c.x2), r, c.x1), r, c.x0);
-    const f2 Y = fma2(fma2(fma2(bc(c.y3), r, c.y2), r, c.y1), r, c.y0);
+    const f2 X = fma2(fma2(bc(c.x2), r, c.x1), r, c.x0);        // the r^3 terms (< 3e-6 relative, 1e-8 absolute) are dropped
+    const f2 Y = fma2(fma2(bc(c.y2), r, c.y1), r, c.y0);
     sr = fma2(r, X, sr);
     si = fma2(mul2(v, r), Y, si);
 }
@@ -178,14 +177,14 @@ MEDEV FarCoef far_load(const float4* p, int stride) {
     const unsigned ax = (unsigned)__cvta_generic_to_shared(p), ay = (unsigned)__cvta_generic_to_shared(p + stride);
     // "memory": the compiler must not sink or drop far_store's plain stores, which only these loads read
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(ax) : "memory");
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(y.x), "=f"(y.y), "=f"(y.z), "=f"(y.w) : "r"(ay) : "memory");
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(y.x), "=f"(y.y) : "r"(ay) : "memory");
     FarCoef c;
-    c.x3 = x.x; c.x2 = x.y; c.x1 = x.z; c.x0 = x.w; c.y3 = y.x; c.y2 = y.y; c.y1 = y.z; c.y0 = y.w;
+    c.x2 = x.x; c.x1 = x.y; c.x0 = x.z; c.y2 = x.w; c.y1 = y.x; c.y0 = y.y;
     return c;
 }
 MEDEV void far_store(float4* p, int stride, const FarCoef& c) {
-    p[0] = make_float4(c.x3, c.x2, c.x1, c.x0);
-    p[stride] = make_float4(c.y3, c.y2, c.y1, c.y0);
+    p[0] = make_float4(c.x2, c.x1, c.x0, c.y2);
+    *reinterpret_cast<float2*>(p + stride) = make_float2(c.y1, c.y0);
 }
 
 // Core region (Weideman).  D = 1/(L - iz) = r ((L+a) + i v), r = 1/|L - iz|^2, Z = (L + iz) D.  With t = 2 Re Z,
@@ -324,8 +323,8 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
                     const f2 vc = add2(v, bc(-d.shift[c] * vB));
                     const f2 rr_ = rcp2(fma2(vc, vc, fad.a2));                        // 1 / |z|^2
                     const f2 rw = mul2(d.weight[c], rr_);                             // weight_c / |z|^2
-                    const f2 X = fma2(fma2(fma2(bc(far.x3), rr_, far.x2), rr_, far.x1), rr_, far.x0);
-                    const f2 Y = fma2(fma2(fma2(bc(far.y3), rr_, far.y2), rr_, far.y1), rr_, far.y0);
+                    const f2 X = fma2(fma2(bc(far.x2), rr_, far.x1), rr_, far.x0);
+                    const f2 Y = fma2(fma2(bc(far.y2), rr_, far.y1), rr_, far.y0);
                     ar = fma2(rw, X, ar);
                     ai = fma2(mul2(vc, rw), Y, ai);
                 }
