@@ -23,16 +23,16 @@ if ROOT not in sys.path:
 from paper_1208_0302_b200 import workloads as W  # noqa: E402
 
 # FP32 work per wavelength point of the fused fitness loop = EXECUTED flop of the current kernel, counted from the ncu
-# source page of a capture of the config1 shape (profiles/r1f_ga_invert_ncu.md: predicated-on thread instructions per
+# source page of a capture of the config1 shape (profiles/r1h_ga_invert_ncu.md: predicated-on thread instructions per
 # SASS opcode / lambda-points; FFMA2 = 4 flop, FMUL2 / FADD2 / FFMA = 2, FMUL / FADD = 1).  It is re-counted whenever the
-# kernel changes (r1a: 477, r1b: 280, r1c: 265.7, r1f: 263.3), so `frac` is the FP32-pipe utilisation, not an inflated textbook
+# kernel changes (r1a: 477, r1b: 280, r1c: 265.7, r1f: 263.3, r1h: 237.6), so `frac` is the FP32-pipe utilisation, not an inflated textbook
 # count.  See DESIGN.md "Measurement".  config0 (one line) is not the bench default and carries an estimate.
-FLOP_PER_POINT = {"config0_tiny": 150.0, "config1_map256": 263.3, "config3_fulldisc": 263.3, "config4_stress11": 264.0}
+FLOP_PER_POINT = {"config0_tiny": 140.0, "config1_map256": 237.6, "config3_fulldisc": 237.6, "config4_stress11": 238.3}
 # MUFU (SFU / XU pipe) instructions per wavelength point, same capture: 6 Voigt reciprocals + 1 for the determinant (+ 1 for the
 # field-free profile of the 11-parameter model)
 MUFU_PER_POINT = 7.13
 # DRAM traffic of ga_invert_kernel per pixel, from the same capture (dram__bytes_read.sum + write.sum) / pixels
-DRAM_BYTES_PER_PIXEL_NCU = 8.496128e6 / 4096      # at L = 128 (2088 algorithmic bytes); scaled by 16 L + 40 for other grids
+DRAM_BYTES_PER_PIXEL_NCU = 8.528128e6 / 4096      # at L = 128 (2088 algorithmic bytes); scaled by 16 L + 40 for other grids
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 
 
