@@ -160,11 +160,12 @@ MEDEV FarCoef far_coef(float a, float strength) {
     return c;
 }
 
-// accumulates r_l w(v + i a) into (sr, si)
+// accumulates r_l w(v + i a) into (sr, si); LINEAR: beyond |z| = 20 the r^2 terms are dropped too
+template <bool LINEAR>
 MEDEV void faddeeva_far_acc(f2 v, f2 r2, const FarCoef& c, f2& sr, f2& si) {
     const f2 r = rcp2(r2);
-    const f2 X = fma2(fma2(bc(c.x2), r, c.x1), r, c.x0);        // the r^3 terms (< 3e-6 relative, 1e-8 absolute) are dropped
-    const f2 Y = fma2(fma2(bc(c.y2), r, c.y1), r, c.y0);
+    const f2 X = LINEAR ? fma2(bc(c.x1), r, c.x0) : fma2(fma2(bc(c.x2), r, c.x1), r, c.x0);   // r^3 terms dropped (< 1e-8 abs)
+    const f2 Y = LINEAR ? fma2(bc(c.y1), r, c.y0) : fma2(fma2(bc(c.y2), r, c.y1), r, c.y0);
     sr = fma2(r, X, sr);
     si = fma2(mul2(v, r), Y, si);
 }
@@ -285,9 +286,15 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
         // straight-line code that the scheduler interleaves; the series shortens with distance from the line.
         if (rmin >= far2) {
             const FarCoef far = FARS ? far_load(far_s + 2 * l * far_stride, far_stride) : far_r;
-            faddeeva_far_acc(v, r2p, far, pr, pi);
-            faddeeva_far_acc(vb, r2b, far, br, bi);
-            faddeeva_far_acc(vr, r2r, far, rr, ri);
+            if (rmin >= 400.0f) {
+                faddeeva_far_acc<true>(v, r2p, far, pr, pi);
+                faddeeva_far_acc<true>(vb, r2b, far, br, bi);
+                faddeeva_far_acc<true>(vr, r2r, far, rr, ri);
+            } else {
+                faddeeva_far_acc<false>(v, r2p, far, pr, pi);
+                faddeeva_far_acc<false>(vb, r2b, far, br, bi);
+                faddeeva_far_acc<false>(vr, r2r, far, rr, ri);
+            }
             return;
         }
         if (rmin >= FAD_FAR2) {                                   // a > FAD_FAR_AMAX: the series itself
