@@ -23,16 +23,18 @@ if ROOT not in sys.path:
 from paper_1208_0302_b200 import workloads as W  # noqa: E402
 
 # FP32 work per wavelength point of the fused fitness loop = EXECUTED flop of the current kernel, counted from the ncu
-# source page of a capture of the config1 shape (profiles/r1h_ga_invert_ncu.md: predicated-on thread instructions per
+# source page of a capture of the config1 shape (profiles/r1i_ga_invert_ncu.md: predicated-on thread instructions per
 # SASS opcode / lambda-points; FFMA2 = 4 flop, FMUL2 / FADD2 / FFMA = 2, FMUL / FADD = 1).  It is re-counted whenever the
-# kernel changes (r1a: 477, r1b: 280, r1c: 265.7, r1f: 263.3, r1h: 237.6), so `frac` is the FP32-pipe utilisation, not an inflated textbook
+# kernel changes (r1a: 477, r1b: 280, r1c: 265.7, r1f: 263.3, r1h: 237.6, r1i: 218.8), so `frac` is the FP32-pipe utilisation, not an inflated textbook
 # count.  See DESIGN.md "Measurement".  config0 (one line) is not the bench default and carries an estimate.
-FLOP_PER_POINT = {"config0_tiny": 140.0, "config1_map256": 237.6, "config3_fulldisc": 237.6, "config4_stress11": 238.3}
+FLOP_PER_POINT = {"config0_tiny": 130.0, "config1_map256": 218.8, "config3_fulldisc": 218.8, "config4_stress11": 219.5}
+# fraction of cycles the FMA pipe was busy in that capture (sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed)
+FMA_PIPE_BUSY_NCU = 0.695
 # MUFU (SFU / XU pipe) instructions per wavelength point, same capture: 6 Voigt reciprocals + 1 for the determinant (+ 1 for the
 # field-free profile of the 11-parameter model)
 MUFU_PER_POINT = 7.13
 # DRAM traffic of ga_invert_kernel per pixel, from the same capture (dram__bytes_read.sum + write.sum) / pixels
-DRAM_BYTES_PER_PIXEL_NCU = 8.528128e6 / 4096      # at L = 128 (2088 algorithmic bytes); scaled by 16 L + 40 for other grids
+DRAM_BYTES_PER_PIXEL_NCU = 8.500224e6 / 4096      # at L = 128 (2088 algorithmic bytes); scaled by 16 L + 40 for other grids
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 
 
@@ -384,7 +386,7 @@ def run_b200(args):
             "syntheses_per_s": value * syn, "median_chi2": med_chi2,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": DRAM_BYTES_PER_PIXEL_NCU * n_active * (16 * L + 40) / 2088.0, "algorithmic_bytes": (16 * L + 40) * n_active,
-                         "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt,
+                         "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt, "fma_pipe_busy_ncu": FMA_PIPE_BUSY_NCU,
                          "peak_measured_ffma_tflops": probe["ffma"]["tflops"],
                          "mufu_per_s_measured": probe["mufu"]["thread_inst_per_s"],
                          "sfu": {"mufu_per_lambda_point": MUFU_PER_POINT, "achieved_per_s": MUFU_PER_POINT * points_per_launch / launch_s,
