@@ -167,3 +167,20 @@ def test_fused_fitness_vs_oracle(B, which):
     rel = np.abs(got - want) / want
     assert rel.max() < 2e-4, rel.max()
     assert np.median(rel) < 1e-5
+
+
+def test_me_synth_large_damping(B):
+    # damping beyond the configs' box: a in (0.5, 0.75] still takes the far-tier polynomials (FAD_FAR_AMAX), a > 0.75 the
+    # plain wing series; both must hold the synthesis tolerance, also at the largest eta0
+    c1 = W.config1()
+    lam = c1["lam"]
+    P = 3000
+    p = W.draw_truth(P, seed=55, b_lo=1.0, b_hi=3500.0)
+    rng = np.random.default_rng(9)
+    p[:, 5] = np.concatenate([rng.uniform(0.5, 0.75, P // 3), rng.uniform(0.75, 0.76, P // 3), rng.uniform(0.76, 2.5, P - 2 * (P // 3))])
+    p[::2, 3] = 50.0
+    ln = oracle_lines(c1["lines"], True)
+    ref = orc.synth(p, lam, ln, threads=NTHREADS)
+    out, _ = B.me_synth(dev(p), lam, B.line_data_from_workload(c1["lines"], True))
+    err = np.abs(out.cpu().numpy() - ref) / (p[:, 7] + p[:, 8])[:, None, None]
+    assert err.max() <= 2e-5, (err.max(), p[np.unravel_index(err.argmax(), err.shape)[0]])
