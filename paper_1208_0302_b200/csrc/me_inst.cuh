@@ -192,7 +192,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 template <int NL, bool TRIPLET, int M>
 __global__ void __launch_bounds__(SYNTH_THREADS, 4)
 me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
-                int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
+                const int* __restrict__ perm, int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
                 float w2I, float w2Q, float w2U, float w2V, float inv_nu, float* __restrict__ out_chi2) {
     extern __shared__ float4 smem4[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -202,7 +202,8 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
     for (int64_t base = (int64_t)blockIdx.x * SYNTH_THREADS; base < P; base += (int64_t)gridDim.x * SYNTH_THREADS) {
         const int64_t wbase = base + warp * 32;                 // first vector of this warp
         if (wbase >= P) continue;
-        const int64_t v = wbase + lane < P ? wbase + lane : P - 1;   // idle lanes recompute the last vector, never store
+        const int64_t slot = wbase + lane < P ? wbase + lane : P - 1;   // idle lanes recompute the last vector, never store
+        const int64_t v = perm != nullptr ? (int64_t)__ldg(perm + slot) : slot;   // processing order -> vector (synth_order_kernel)
         float p[M];
 #pragma unroll
         for (int j = 0; j < M; ++j) p[j] = __ldg(params + v * M + j);
@@ -239,8 +240,9 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
 #pragma unroll 4
                     for (int it = 0; it < 16; ++it) {
                         const int row = 8 * it + (lane >> 2), lv = row >> 2, st = row & 3;
+                        const int64_t vv = __shfl_sync(0xffffffffu, v, lv);
                         if (lv < nvec && q < ncol)
-                            __stcs(reinterpret_cast<float4*>(out_stokes + ((wbase + lv) * 4 + st) * (int64_t)L + 2 * jp0 + q),
+                            __stcs(reinterpret_cast<float4*>(out_stokes + (vv * 4 + st) * (int64_t)L + 2 * jp0 + q),
                                    *reinterpret_cast<const float4*>(tile + lv * SYNTH_VS + st * SYNTH_CW + q));
                     }
                 } else {
@@ -248,8 +250,9 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
 #pragma unroll 4
                     for (int it = 0; it < 64; ++it) {
                         const int row = 2 * it + (lane >> 4), lv = row >> 2, st = row & 3;
+                        const int64_t vv = __shfl_sync(0xffffffffu, v, lv);
                         if (lv < nvec && k < ncol)
-                            __stcs(out_stokes + ((wbase + lv) * 4 + st) * (int64_t)L + 2 * jp0 + k, tile[lv * SYNTH_VS + st * SYNTH_CW + k]);
+                            __stcs(out_stokes + (vv * 4 + st) * (int64_t)L + 2 * jp0 + k, tile[lv * SYNTH_VS + st * SYNTH_CW + k]);
                     }
                 }
                 __syncwarp();
@@ -494,7 +497,7 @@ cudaError_t ME_INST_NAME(launch_uncertainty)(const SynthDesc& sd, const GaDesc& 
     return cudaGetLastError();
 }
 
-cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params, const float* mu, int64_t P,
+cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params, const float* mu, const int* perm, int64_t P,
                                        float* out_stokes, const float* obs_ref, const float* w2, float inv_nu,
                                        float* out_chi2, cudaStream_t st) {
     int dev = 0, sms = 148;
@@ -504,7 +507,7 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
     const int64_t cap = (int64_t)sms * 4;                            // persistent grid: 4 resident blocks per SM
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
     const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float);
-    me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, P, out_stokes, obs_ref, w2[0],
+    me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, perm, P, out_stokes, obs_ref, w2[0],
                                                                                    w2[1], w2[2], w2[3], inv_nu, out_chi2);
     return cudaGetLastError();
 }

@@ -184,3 +184,29 @@ def test_me_synth_large_damping(B):
     out, _ = B.me_synth(dev(p), lam, B.line_data_from_workload(c1["lines"], True))
     err = np.abs(out.cpu().numpy() - ref) / (p[:, 7] + p[:, 8])[:, None, None]
     assert err.max() <= 2e-5, (err.max(), p[np.unravel_index(err.argmax(), err.shape)[0]])
+
+
+def test_me_synth_large_batch_order_is_invisible(B):
+    # batches of >= 400 000 vectors are visited in a counting-sort order (tier coherence); every output must sit at its own
+    # index and be bit-identical to what the same vector gives in a small (unsorted) batch, with and without chi2
+    c1 = W.config1()
+    lam = c1["lam"]
+    P = 400003
+    p = W.draw_truth(P, seed=91, b_lo=1.0, b_hi=3500.0)
+    p[:5, 0] = 0.0                                              # B = 0 and extreme keys
+    p[5:10, 6] = [-30.0, 30.0, -7.99, 7.99, 0.0]
+    mu = np.random.default_rng(4).uniform(0.05, 1.0, P)
+    ld = B.line_data_from_workload(c1["lines"], True)
+    d_p, d_mu = dev(p), dev(mu)
+    obs_ref = dev(orc.synth(p[:1], lam, oracle_lines(c1["lines"], True))[0])
+    wos = c1["ga"]["stokes_weight"] / c1["ga"]["sigma"]
+    big, chi_big = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos)
+    for s in (0, 150000, 300000):
+        e = min(s + 150000, P)
+        small, chi_small = B.me_synth(d_p[s:e].contiguous(), lam, ld, mu=d_mu[s:e].contiguous(), obs_ref=obs_ref, w_over_sigma=wos)
+        assert torch.equal(big[s:e], small) and torch.equal(chi_big[s:e], chi_small)
+    # and a sample against the oracle
+    idx = np.arange(0, P, 4000)
+    ref = orc.synth(p[idx], lam, oracle_lines(c1["lines"], True), mu=mu[idx], threads=NTHREADS)
+    err = np.abs(big.cpu().numpy()[idx] - ref) / (p[idx, 7] + mu[idx] * p[idx, 8])[:, None, None]
+    assert err.max() <= 2e-5
