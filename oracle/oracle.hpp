@@ -13,13 +13,18 @@
 // Parity pins (tests/test_oracle_*.py, -m "not gpu"):
 //   faddeeva       pinned  (erfc / Dawson closed forms, scipy.special.wofz, ODE w' = -2zw + 2i/sqrt(pi))
 //   zeeman_pattern pinned  (Table 1 g_eff, 12 components for 6301.5, centre-of-gravity identity)
-//   synth          pinned  (B=0 and gamma=0 closed forms, 4x4 solve of eq. 12, symmetries, weak field)
+//   synth          pinned  (B=0 and gamma=0 closed forms, 4x4 solve of eq. 12, symmetries, weak field;
+//                           P12 gamma=90/chi=0 closed form I+-Q through scipy's wofz fixes the linear-polarisation
+//                           amplitude kL; P13 eta0 -> 0 expansion e - eta0 A e + eta0^2 A^2 e, A built in numpy from the
+//                           LL04 matrix, fixes the signs of rho_Q, rho_U, rho_V and of K: both fail when kL is halved
+//                           or the .imag() terms are negated)
 //   chi2           pinned  (expected value at truth, brute-force grid minimum)
 //   philox4x32_10  pinned  (published known-answer vectors of Salmon et al. 2011)
 //   synth_n (11 parameters, reading F13) pinned (alpha=1,s=0 -> synth; alpha=0 -> B=0 closed form; s=1 -> I_fixed;
 //                  Q,U,V scale with (1-s) alpha; bilinearity in alpha and s)
 //   uncertainty    pinned  (exact Hessian of quadratic / quartic test functions, closed-form inverse; noise scaling)
-//   ga             operators pinned by brute-force re-derivation in Python on tiny inputs and by
+//   ga             operators pinned by brute-force re-derivation in Python on tiny inputs (both variants, incl. the
+//                  member-index rule of variant-1 tournaments inside and outside restart generations) and by
 //                  invariants; absolute recovery accuracy: PARITY UNPINNED (the paper prints no
 //                  reproducible recovery numbers, Table 4 PAPER.md:340-345 is for SOLIS data).
 #pragma once

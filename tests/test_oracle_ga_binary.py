@@ -158,3 +158,56 @@ def test_binary_variant_inversion_converges_and_is_deterministic():
     model = orc.synth(a["params"], lam, ln)
     chk = [orc.chi2(o, m, cfg["stokes_weight"], cfg["sigma"]) for o, m in zip(obs, model)]
     assert np.allclose(chk, a["chi2"], rtol=1e-12)
+
+
+def test_binary_step_transcription_from_raw_philox_words():
+    """An independent numpy transcription of readings V2-V5 from raw Philox words (orc.philox is KAT-pinned): which MEMBER
+    a tournament draw names — floor(u P) itself outside restart generations (reading V3 = G3), order[floor(u n_live)]
+    at a restart (reading V2) — the pair keying, the bit-mask crossover, the LSB-biased mutation and the fresh points."""
+    pop, G, seed, base, k = 10, 8, 77, 5, 3                                 # N_samp = 2: t = 2, 4, 6 restart
+    cfg = _cfg(pop, gens=G, tournament_k=k)
+    rng = np.random.default_rng(8)
+    genes = np.rint(rng.random((2, pop, M)) * 65535).astype(np.float32)
+    chi2v = rng.random((2, pop)) + 0.5
+    chi2v[1, 6] = chi2v[1, 2]                                               # a tie: lower index wins
+    f32 = np.float32
+    u01 = lambda x: f32(int(x) >> 8) * f32(2.0 ** -24)
+    below = lambda x, n: ((int(x) >> 8) * n) >> 24
+    for t in (1, 2, 3, 4, G):
+        restart = (t % 2 == 0) and t < G
+        n_live = pop - pop // 2 if restart else pop
+        got = orc.ga_step(genes, chi2v, t, cfg, seed=seed, pixel_base=base).astype(np.uint32)
+        for n in range(2):
+            order = sorted(range(pop), key=lambda q: (chi2v[n, q], q))
+            want = np.empty((pop, M), dtype=np.uint32)
+            want[0] = genes[n, order[0]].astype(np.uint32)
+            sh = np.array([_shift(seed, base + n, j) for j in range(M)], dtype=np.uint32)
+            for i in range(1, pop):
+                if i >= n_live:
+                    idx = pop + (t // 2 - 1) * (pop // 2) + (i - n_live) + 1
+                    want[i] = (orc.sobol(idx, 1, M)[0] >> np.uint32(16)) ^ sh
+                    continue
+                key = 2 * ((i + 1) // 2) - 1
+
+                def tour(block):
+                    r = orc.philox(seed, base + n, t, key, block)
+                    cand = [order[below(r[m], n_live)] if restart else below(r[m], pop) for m in range(k)]
+                    return min(cand, key=lambda q: (chi2v[n, q], q))
+                A, B = tour(0), tour(1)
+                r2 = orc.philox(seed, base + n, t, key, 2)
+                cross = u01(r2[0]) < f32(cfg["p_cross"])
+                cut = 1 + below(r2[1], 16 * M - 1)
+                first, second = (A, B) if i & 1 else (B, A)
+                for j in range(M):
+                    k1, k2 = int(genes[n, first, j]), int(genes[n, second, j])
+                    kk = k1
+                    if cross:
+                        nhead = min(max(cut - 16 * j, 0), 16)
+                        mask = (0xFFFF << (16 - nhead)) & 0xFFFF
+                        kk = (k1 & mask) | (k2 & ~mask & 0xFFFF)
+                    r = orc.philox(seed, base + n, t, i, 3 + j // 2)
+                    xm, xd = int(r[2 * (j % 2)]), int(r[2 * (j % 2) + 1])
+                    if u01(xm) < f32(cfg["p_mut"]):
+                        kk ^= ((xd & 0xFFFF) & (xd >> 16)) >> (xm & 15)
+                    want[i, j] = kk
+            assert np.array_equal(got[n], want), (t, n)

@@ -173,3 +173,96 @@ def test_P11_brute_force_grid_minimum_is_at_truth():
         c = np.array([orc.chi2(obs, m, w, sig) for m in models])
         k = int(np.argmin(c))
         assert abs(grid[k, 0] - p[0]) < 1e-9 and abs(grid[k, 1] - p[1]) < 1e-9 and c[k] < 1e-20
+
+
+def _profiles_numpy(p, lam, lines):
+    """phi_k + i psi_k (k = blue, pi, red) from scipy's wofz: reading F2, written here from SURVEY.md 8(c) steps 1-2."""
+    prof = {-1: 0j, 0: 0j, 1: 0j}
+    for l in lines:
+        dld = p[4] * 1e-3 * l["lambda0"] / l["lambda_ref"]
+        v = ((lam - l["lambda0"]) - l["lambda0"] * p[6] / C_KMS) / dld
+        vB = ZEEMAN * l["lambda0"] ** 2 * p[0] / dld
+        for s, wgt, k in zip(l["shift"], l["weight"], l["kind"]):
+            prof[k] = prof[k] + l["strength"] * wgt * special.wofz(v - s * vB + 1j * p[5]) / SQPI
+    return prof[-1], prof[0], prof[1]
+
+
+def test_P12_transverse_field_closed_form_pins_linear_amplitude():
+    """gamma = 90 deg, chi = 0: K splits into the (I,Q) block [[eI,eQ],[eQ,eI]] and the (U,V) block, so
+    I+Q = S0 + mu S1/(eI+eQ), I-Q = S0 + mu S1/(eI-eQ); the textbook transverse Zeeman effect says light polarised
+    ALONG the field sees only the pi component, light polarised ACROSS it the mean of the sigma components:
+    eI+eQ = 1 + eta0 phi_p, eI-eQ = 1 + eta0 (phi_b+phi_r)/2 (eq. 8, 12 PAPER.md:185-187, 204-216; reading F1).
+    Fixes the factor of the linear-polarisation amplitude kL in oracle/synth.cpp."""
+    mu = 0.7
+    cases = [([dict(lambda0=6302.5017, strength=1.0, shift=[0.0, -2.5, 2.5], weight=[1, 1, 1], kind=[0, -1, 1],
+                    lambda_ref=6302.5017)], W.grid(6302.5017, 81, 0.012))]
+    cfg = W.config1()
+    two = []
+    for l in cfg["lines"]:
+        g = l["g_eff"]
+        two.append(dict(lambda0=l["lambda0"], strength=l["strength"], shift=[0.0, -g, g], weight=[1, 1, 1],
+                        kind=[0, -1, 1], lambda_ref=W.LAMBDA_REF))
+    cases.append((two, cfg["lam"]))
+    for lines, lam in cases:
+        ln = orc.Lines([{k: v for k, v in l.items() if k != "lambda_ref"} for l in lines], lines[0]["lambda_ref"])
+        for p in _draws(12, seed=31):
+            p = p.copy(); p[1] = 90.0; p[2] = 0.0
+            out = orc.synth(p, lam, ln, mu=[mu])[0]
+            pb, pp, pr = _profiles_numpy(p, lam, lines)
+            Ipar = p[7] + mu * p[8] / (1.0 + p[3] * pp.real)
+            Iperp = p[7] + mu * p[8] / (1.0 + p[3] * 0.5 * (pb.real + pr.real))
+            assert np.max(np.abs(out[0] + out[1] - Ipar)) < 1e-12
+            assert np.max(np.abs(out[0] - out[1] - Iperp)) < 1e-12
+            # U and V vanish up to cos(90 deg) = 6e-17 in double
+            assert np.max(np.abs(out[2])) < 1e-15 and np.max(np.abs(out[3])) < 1e-15
+            assert np.max(np.abs(out[1])) > 1e-4                  # not trivially satisfied
+
+
+def test_P13_weak_line_expansion_pins_magneto_optical_signs():
+    """eta0 -> 0: K = 1 + eta0 A (eq. 8) gives K^-1 e = e - eta0 A e + eta0^2 A^2 e - ...  The first-order term holds only
+    the absorption profiles (phi); the magneto-optical profiles (psi = Im w / sqrt(pi), reading F3) enter FIRST at second
+    order, e.g. at chi = 0: (A^2 e)_U = aQ' rV' ... = rQ aV - rV aQ.  A is built here in numpy from the matrix of SURVEY.md
+    8(c) step 5 (the LL04 form the paper cites) with scipy's wofz; the oracle's profile is compared order by
+    order.  Fixes the sign with which Im(kL), Im(kV) enter rho_Q, rho_U, rho_V in oracle/synth.cpp and the sign convention
+    of K in stokes_by_solve / stokes_closed_form (eq. 12-13)."""
+    lam0, g = 6302.5017, 2.5
+    lines = [dict(lambda0=lam0, strength=1.0, shift=[0.0, -g, g], weight=[1, 1, 1], kind=[0, -1, 1], lambda_ref=lam0)]
+    ln = single_line(g, lam0)
+    lam = W.grid(lam0, 61, 0.015)
+    eta0, mu = 1e-4, 0.9
+    seen_u = 0
+    for p, chi in zip(_draws(12, seed=41), [0.0, 0.0, 0.0, 0.0, 20.0, 65.0, 100.0, 140.0, 0.0, 33.0, 90.0, 170.0]):
+        p = p.copy(); p[0] = max(p[0], 600.0); p[2] = chi; p[3] = eta0
+        p[1] = min(max(p[1], 25.0), 155.0)
+        if abs(p[1] - 90.0) < 10.0:
+            p[1] = 60.0                                           # keep both eta_V and eta_Q away from zero
+        out = orc.synth(p, lam, ln, mu=[mu])[0]
+        x = out / (mu * p[8]); x[0] -= p[7] / (mu * p[8])         # K^-1 e
+        pb, pp, pr = _profiles_numpy(p, lam, lines)
+        gam, ch = math.radians(p[1]), math.radians(p[2])
+        s2, c2 = math.sin(gam) ** 2, math.cos(gam) ** 2
+        kI = 0.5 * (pp * s2 + 0.5 * (pb + pr) * (1 + c2))
+        kL = 0.5 * (pp - 0.5 * (pb + pr)) * s2
+        kV = 0.5 * (pr - pb) * math.cos(gam)
+        aI, aQ, aU, aV = kI.real, kL.real * math.cos(2 * ch), kL.real * math.sin(2 * ch), kV.real
+        rQ, rU, rV = kL.imag * math.cos(2 * ch), kL.imag * math.sin(2 * ch), kV.imag
+        for j in range(lam.size):
+            A = np.array([[aI[j], aQ[j], aU[j], aV[j]],
+                          [aQ[j], aI[j], rV[j], -rU[j]],
+                          [aU[j], -rV[j], aI[j], rQ[j]],
+                          [aV[j], rU[j], -rQ[j], aI[j]]])
+            e = np.array([1.0, 0.0, 0.0, 0.0])
+            first, second = -A @ e, A @ A @ e
+            got1 = (x[:, j] - e) / eta0
+            got2 = (x[:, j] - e - eta0 * first) / eta0 ** 2
+            assert np.max(np.abs(got1 - first)) < 3e-4 * np.max(np.abs(A)) + 1e-12
+            assert np.max(np.abs(got2 - second)) < 2e-3 * np.max(np.abs(second)) + 1e-7
+        if chi == 0.0:
+            # the magneto-optical cross term alone: U(chi = 0) = mu S1 eta0^2 (rQ aV - rV aQ), sign included
+            U2 = mu * p[8] * eta0 ** 2 * (rQ * aV - rV * aQ)
+            big = np.abs(U2) > 0.2 * np.max(np.abs(U2))
+            assert np.max(np.abs(U2)) > 1e-12
+            assert np.all(np.sign(out[2][big]) == np.sign(U2[big]))
+            assert np.max(np.abs(out[2] - U2)) < 2e-3 * np.max(np.abs(U2))
+            seen_u += 1
+    assert seen_u >= 4
