@@ -40,7 +40,10 @@ def prior_box(b_lo=10.0, b_hi=3000.0, npar=NPAR):
 
 
 def mutation_schedule(generations, s0=0.5, s_end=0.0025):
-    """Reading G3: s_t = s0 (s_end/s0)^(t/G), tabulated in double and rounded to binary32, t = 0..G."""
+    """Reading G3: s_t = s0 (s_end/s0)^(t/G), tabulated in double and rounded to binary32, t = 0..G.  s0 and s_end are
+    the binary32 values the C ABI carries (ga_cfg.mut_scale0 / mut_scale_end), so that the table the library builds itself
+    when ga_cfg.mut_scale_table is NULL is this table."""
+    s0, s_end = float(np.float32(s0)), float(np.float32(s_end))
     t = np.arange(generations + 1, dtype=np.float64)
     return (s0 * (s_end / s0) ** (t / max(generations, 1))).astype(np.float32)
 

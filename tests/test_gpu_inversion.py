@@ -272,3 +272,36 @@ def test_maximum_sizes(B):
             B.ga_invert(dev(o0), c0["lam"], B.line_data_from_workload(c0["lines"], True), bad, 6)
     with pytest.raises(B.MeError):
         B.me_synth(dev(t0), W.grid(6302.5, 513, 0.01), B.line_data_from_workload(c0["lines"], True))
+
+
+def test_library_built_mutation_schedule_equals_the_table(B):
+    # "geometric schedule, table built on host".  A C caller that leaves ga_cfg.mut_scale_table NULL gets the
+    # schedule the library builds from mut_scale0 / mut_scale_end (std::pow in double, rounded to binary32); it must be the
+    # table both sides are otherwise handed (workloads.mutation_schedule, reading G3), or GPU and oracle trajectories part.
+    # Called through ctypes directly: the binding always passes the table.
+    import ctypes as C
+    c0 = W.config0()
+    N = 24
+    truth, obs, ln = make_obs(c0, N, threads=NTHREADS)
+    ld = B.line_data_from_workload(c0["lines"], True)
+    d_obs = dev(obs)
+    lam = np.ascontiguousarray(c0["lam"], dtype=np.float64)
+    sig = np.ascontiguousarray(c0["ga"]["sigma"], dtype=np.float32)
+    outs = []
+    for use_table in (True, False):
+        c, keep = B.make_ga_cfg(c0["ga"])
+        if not use_table:
+            c.mut_scale_table = C.POINTER(C.c_float)()             # NULL
+        p = torch.empty((N, 9), dtype=torch.float32, device="cuda")
+        x = torch.empty((N,), dtype=torch.float32, device="cuda")
+        rc = B.lib().ga_invert(C.c_void_p(d_obs.data_ptr()), C.c_int64(N), C.c_void_p(0), sig.ctypes.data_as(C.POINTER(C.c_float)),
+                               lam.ctypes.data_as(C.POINTER(C.c_double)), C.c_int(lam.size), C.byref(ld.c), C.byref(c),
+                               C.c_uint64(W.SEED_GA), C.c_void_p(p.data_ptr()), C.c_void_p(x.data_ptr()),
+                               C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        assert rc == 0, rc
+        torch.cuda.synchronize()
+        outs.append((p.cpu().numpy(), x.cpu().numpy()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])     # bit-identical
+    # and the table path is the oracle's trajectory
+    res = orc.ga_invert(obs, c0["lam"], ln, c0["ga"], seed=W.SEED_GA, threads=NTHREADS)
+    assert np.mean(np.abs(outs[1][1] - res["chi2"]) <= 2e-4 * res["chi2"]) >= 0.85

@@ -150,3 +150,30 @@ def test_config4_launch_configuration_sampled(B):
     same = np.abs(gc - res["chi2"]) <= 2e-4 * res["chi2"]
     assert same.mean() >= 0.75, (same.mean(), gc, res["chi2"])
     assert np.all(np.abs(gc - res["chi2"]) <= 0.25 * res["chi2"])
+
+
+def test_config4_full_depth_sampled(B):
+    # BASELINE config 4 at its OWN depth: L = 256, pop 512 (512-thread CTAs), 11 genes, all 300 generations, on 8 pixels
+    # under global ids of the 512^2 map (the oracle needs ~150 core-seconds per pixel; the 8 run in parallel).  After 300
+    # generations both sides sit at the noise floor of the same noise realisation, so chi2 agrees pixel by pixel even
+    # where the binary32-vs-binary64 `<` (reading G4) has parted the trajectories.
+    c4 = W.config4()
+    ln, nm, ld = _setup(B, c4["lines"], True, c4["lam"])
+    N, base = 8, 131072
+    ga = c4["ga"]
+    assert ga["pop"] == 512 and ga["generations"] == 300
+    truth = W.draw_truth(N, seed=78, b_lo=1.0, b_hi=500.0, npar=11)
+    clean = orc.synth(truth, c4["lam"], ln, nm_profile=nm, threads=NTHREADS)
+    obs = (clean + W.draw_noise(clean.shape, 3e-3, stream=5)).astype(np.float32).astype(np.float64)
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(min(N, NTHREADS)) as ex:             # one oracle call per pixel id; ctypes releases the GIL
+        rs = list(ex.map(lambda i: orc.ga_invert(obs[i:i + 1], c4["lam"], ln, ga, seed=W.SEED_GA, nm_profile=nm,
+                                                 pixel_base=base + i, threads=1), range(N)))
+    oc = np.array([r["chi2"][0] for r in rs])
+    gp, gc = B.ga_invert(dev(obs), c4["lam"], ld, ga, W.SEED_GA, pixel_id_base=base)
+    gc = gc.cpu().numpy().astype(np.float64)
+    same = np.abs(gc - oc) <= 2e-4 * oc
+    print("config4 full depth: identical-optimum fraction %.2f, max |dchi2|/chi2 %.3g" % (same.mean(), np.max(np.abs(gc - oc) / oc)))
+    assert np.all(np.isfinite(gc))
+    assert abs(np.median(gc) - np.median(oc)) <= 0.01 * np.median(oc), (np.median(gc), np.median(oc))
+    assert np.all(np.abs(gc - oc) <= 0.10 * oc), (gc, oc)
