@@ -28,6 +28,7 @@
 #ifndef ME_B200_H
 #define ME_B200_H
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -77,10 +78,24 @@ typedef struct {
  *   lambda_grid_A host [L] f64 (Angstrom)    out_stokes  device [P, 4, L] f32 or NULL
  *   obs_ref       device [4, L] f32 or NULL  w_over_sigma host [4] f32 (w_s / sigma_s of eq. 16) or NULL
  *   out_chi2      device [P] f32 or NULL: chi2 of each vector against obs_ref, nu = 4L - n_params.
- * At least one of out_stokes / out_chi2 must be given; out_chi2 requires obs_ref and w_over_sigma. P = 0 is a no-op. */
+ * At least one of out_stokes / out_chi2 must be given; out_chi2 requires obs_ref and w_over_sigma. P = 0 is a no-op.
+ * me_synth allocates nothing: the vectors are visited in index order. */
 int me_synth(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
              const me_line_data* line_data, float* out_stokes,
              const float* obs_ref, const float* w_over_sigma, float* out_chi2, void* stream);
+
+/* The same with an optional caller-provided DEVICE workspace ("no allocation visible to the caller
+ * except an optional caller-provided workspace").  With workspace_bytes >= me_synth_workspace_bytes(P) (and that size
+ * non-zero) the vectors are visited in the order of a counting sort on a coarse key of (dlambdaD, v_los, B), which keeps the
+ * lanes of a warp on the same Voigt tiers; every output stays at its own index and is bit-identical to me_synth's.
+ * workspace = NULL or too small: exactly me_synth.  The workspace is scratch: owned by the caller, 16-byte aligned, not
+ * read after the work enqueued by this call has run; it may be reused by later calls on the same stream.
+ * me_synth_workspace_bytes returns 0 where sorting does not pay (small P) or is not possible (P >= 2^31). */
+size_t me_synth_workspace_bytes(int64_t P);
+int me_synth_ws(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
+                const me_line_data* line_data, float* out_stokes,
+                const float* obs_ref, const float* w_over_sigma, float* out_chi2,
+                void* workspace, size_t workspace_bytes, void* stream);
 
 /* GA configuration (readings G0-G5 in DESIGN.md; the paper leaves the operators' details open). */
 typedef struct {

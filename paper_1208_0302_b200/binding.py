@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libme_b200.so")
 _lib = None
 
-EXPORTS = ["me_synth", "ga_invert", "ga_uncertainty", "ga_step", "ga_fitness", "ga_init", "ga_prologue", "me_philox", "me_philox_many", "me_faddeeva",
+EXPORTS = ["me_synth", "me_synth_ws", "me_synth_workspace_bytes", "ga_invert", "ga_uncertainty", "ga_step", "ga_fitness", "ga_init", "ga_prologue", "me_philox", "me_philox_many", "me_faddeeva",
            "me_zeeman_pattern", "me_peak_probe", "me_strerror", "me_last_cuda_error", "me_version"]
 
 
@@ -60,6 +60,8 @@ def lib():
         l.me_strerror.restype = C.c_char_p
         l.me_last_cuda_error.restype = C.c_char_p
         l.me_strerror.argtypes = [C.c_int]
+        l.me_synth_workspace_bytes.restype = C.c_size_t
+        l.me_synth_workspace_bytes.argtypes = [C.c_int64]
         _lib = l
     return _lib
 
@@ -160,8 +162,16 @@ def _grid(lam):
     return lam, lam.ctypes.data_as(C.POINTER(C.c_double)), C.c_int(lam.size)
 
 
-def me_synth(params, lam, line_data, mu=None, out_stokes=None, obs_ref=None, w_over_sigma=None, out_chi2=None, want_stokes=True):
-    """params: CUDA f32 [P, line_data.n_params]. Returns (out_stokes [P,4,L] or None, out_chi2 [P] or None)."""
+def me_synth_workspace_bytes(P):
+    return int(lib().me_synth_workspace_bytes(C.c_int64(P)))
+
+
+def me_synth(params, lam, line_data, mu=None, out_stokes=None, obs_ref=None, w_over_sigma=None, out_chi2=None, want_stokes=True,
+             workspace=None):
+    """params: CUDA f32 [P, line_data.n_params]. Returns (out_stokes [P,4,L] or None, out_chi2 [P] or None).
+
+    workspace: a CUDA uint8 tensor of >= me_synth_workspace_bytes(P) bytes for the ordered visit of large batches (me_synth_ws);
+    None = allocate one here from torch's caching allocator when the library asks for one; False = none (plain me_synth)."""
     import torch
     P = params.shape[0]
     assert params.dim() == 2 and params.shape[1] == line_data.n_params
@@ -173,11 +183,17 @@ def me_synth(params, lam, line_data, mu=None, out_stokes=None, obs_ref=None, w_o
         wos = np.ascontiguousarray(w_over_sigma, dtype=np.float32)
         if out_chi2 is None:
             out_chi2 = torch.empty((P,), dtype=torch.float32, device=params.device)
-    _check(lib().me_synth(_dev(params, torch.float32, "params"), C.c_int64(P), _dev(mu, torch.float32, "mu"), lam_p, L,
-                          C.byref(line_data.c), _dev(out_stokes, torch.float32, "out_stokes"),
-                          _dev(obs_ref, torch.float32, "obs_ref"),
-                          wos.ctypes.data_as(C.POINTER(C.c_float)) if wos is not None else None,
-                          _dev(out_chi2, torch.float32, "out_chi2"), _stream()), "me_synth")
+    if workspace is None:
+        need = me_synth_workspace_bytes(P)
+        workspace = torch.empty((need,), dtype=torch.uint8, device=params.device) if need else False
+    ws_bytes = 0 if workspace is False else int(workspace.numel())
+    _check(lib().me_synth_ws(_dev(params, torch.float32, "params"), C.c_int64(P), _dev(mu, torch.float32, "mu"), lam_p, L,
+                             C.byref(line_data.c), _dev(out_stokes, torch.float32, "out_stokes"),
+                             _dev(obs_ref, torch.float32, "obs_ref"),
+                             wos.ctypes.data_as(C.POINTER(C.c_float)) if wos is not None else None,
+                             _dev(out_chi2, torch.float32, "out_chi2"),
+                             _dev(None if workspace is False else workspace, torch.uint8, "workspace"), C.c_size_t(ws_bytes),
+                             _stream()), "me_synth_ws")
     return out_stokes, out_chi2
 
 

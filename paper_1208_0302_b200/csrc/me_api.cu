@@ -182,9 +182,18 @@ const char* me_strerror(int code) {
     }
 }
 
+size_t me_synth_workspace_bytes(int64_t P) { return me::synth_workspace_bytes(P); }
+
 int me_synth(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
              const me_line_data* line_data, float* out_stokes,
              const float* obs_ref, const float* w_over_sigma, float* out_chi2, void* stream) {
+    return me_synth_ws(params, P, mu, lambda_grid_A, L, line_data, out_stokes, obs_ref, w_over_sigma, out_chi2, nullptr, 0, stream);
+}
+
+int me_synth_ws(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
+                const me_line_data* line_data, float* out_stokes,
+                const float* obs_ref, const float* w_over_sigma, float* out_chi2,
+                void* workspace, size_t workspace_bytes, void* stream) {
     if (P < 0) return ME_ERR_SHAPE;
     me::SynthDesc sd;
     int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
@@ -200,7 +209,7 @@ int me_synth(const float* params, int64_t P, const float* mu, const double* lamb
             w2[s] = w_over_sigma[s] * w_over_sigma[s];
         }
     cudaError_t e = me::launch_synth(sd, params, mu, P, out_stokes, obs_ref, w2, (float)(1.0 / (4.0 * L - sd.npar)),
-                                     out_chi2, (cudaStream_t)stream);
+                                     out_chi2, workspace, workspace_bytes, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 

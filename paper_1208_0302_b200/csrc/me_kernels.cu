@@ -218,24 +218,34 @@ __global__ void synth_scatter_kernel(const int* __restrict__ keys, int64_t P, in
         perm[atomicAdd(cursor + keys[v], 1)] = (int)v;
 }
 
+// Bytes of caller-provided scratch the ordered visit needs (keys [P] | perm [P] | histogram [SYNTH_NKEY] ints); 0 = not used.
+size_t synth_workspace_bytes(int64_t P) {
+    if (P < SYNTH_SORT_MIN || P >= 0x7fffffffLL) return 0;
+    return (size_t)(2 * P + SYNTH_NKEY) * sizeof(int);
+}
+
+// work: caller-provided device scratch or nullptr.  Nothing is allocated here; every launch is checked, and a failure of
+// the three ordering passes is returned before the synthesis is enqueued.
 cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* mu, int64_t P, float* out_stokes,
-                         const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, cudaStream_t st) {
-    int* work = nullptr;
+                         const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, void* work_v, size_t work_bytes,
+                         cudaStream_t st) {
     const int* perm = nullptr;
-    if (P >= SYNTH_SORT_MIN && P < 0x7fffffffLL) {                  // worth three light passes over the parameters
-        cudaError_t e = cudaMallocAsync(&work, (size_t)(2 * P + SYNTH_NKEY) * sizeof(int), st);
-        if (e != cudaSuccess) return e;
+    const size_t need = synth_workspace_bytes(P);
+    if (work_v != nullptr && need != 0 && work_bytes >= need) {     // worth three light passes over the parameters
+        int* work = static_cast<int*>(work_v);
         int *keys = work, *pm = work + P, *hist = work + 2 * P;
-        cudaMemsetAsync(hist, 0, SYNTH_NKEY * sizeof(int), st);
+        cudaError_t e = cudaMemsetAsync(hist, 0, SYNTH_NKEY * sizeof(int), st);
+        if (e != cudaSuccess) return e;
         const unsigned g = (unsigned)((P + 255) / 256 < 148 * 16 ? (P + 255) / 256 : 148 * 16);
         synth_hist_kernel<<<g, 256, 0, st>>>(params, sd.npar, P, keys, hist);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
         synth_scan_kernel<<<1, 1024, 0, st>>>(hist);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
         synth_scatter_kernel<<<g, 256, 0, st>>>(keys, P, hist, pm);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
         perm = pm;
     }
-    cudaError_t e = launch_synth_ordered(sd, params, mu, perm, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
-    if (work != nullptr) cudaFreeAsync(work, st);                   // stream-ordered: after the kernels above
-    return e;
+    return launch_synth_ordered(sd, params, mu, perm, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
 }
 
 cudaError_t launch_ga_step(const GaDesc& gd, int npar, const float* genes_in, const float* chi2_in, int64_t N, int t,

@@ -200,7 +200,17 @@ def test_me_synth_large_batch_order_is_invisible(B):
     d_p, d_mu = dev(p), dev(mu)
     obs_ref = dev(orc.synth(p[:1], lam, oracle_lines(c1["lines"], True))[0])
     wos = c1["ga"]["stokes_weight"] / c1["ga"]["sigma"]
-    big, chi_big = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos)
+    # the ordering scratch is the CALLER's: the library reports its size and allocates nothing itself
+    need = B.me_synth_workspace_bytes(P)
+    assert need == (2 * P + 32768) * 4 and B.me_synth_workspace_bytes(399999) == 0 and B.me_synth_workspace_bytes(2 ** 31) == 0
+    big, chi_big = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos,
+                              workspace=torch.empty((need,), dtype=torch.uint8, device="cuda"))
+    plain, chi_plain = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos, workspace=False)   # me_synth proper
+    assert torch.equal(big, plain) and torch.equal(chi_big, chi_plain)
+    short, chi_short = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos,
+                                  workspace=torch.empty((need - 16,), dtype=torch.uint8, device="cuda"))   # too small: ignored
+    assert torch.equal(big, short) and torch.equal(chi_big, chi_short)
+    del plain, short
     for s in (0, 150000, 300000):
         e = min(s + 150000, P)
         small, chi_small = B.me_synth(d_p[s:e].contiguous(), lam, ld, mu=d_mu[s:e].contiguous(), obs_ref=obs_ref, w_over_sigma=wos)
