@@ -3,7 +3,9 @@
 
 A "step" is one pass of the whole hot path over one batch: one `ga_invert` call (observation staging, generation 0,
 G generations of select/crossover/mutate/evaluate, output) over the map of the chosen workload.
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config1|config3|config4|config0] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config3|config1|config4|config0|config2] [--impl reference]
+Default workload: config3, the north_star target (2048 x 2048 full-disc map, 3.14 M on-disc pixels, 200 generations; one step
+takes about a minute on a B200).  config2 times me_synth (forward synthesis of 1e6 prior draws) as the step.
 One JSON line on stdout (rank 0).  See DESIGN.md "Measurement" for every field.
 """
 import argparse
@@ -22,19 +24,10 @@ if ROOT not in sys.path:
 
 from paper_1208_0302_b200 import workloads as W  # noqa: E402
 
-# FP32 work per wavelength point of the fused fitness loop = EXECUTED flop of the current kernel, counted from the ncu
-# source page of a capture of the config1 shape (profiles/r1i_ga_invert_ncu.md: predicated-on thread instructions per
-# SASS opcode / lambda-points; FFMA2 = 4 flop, FMUL2 / FADD2 / FFMA = 2, FMUL / FADD = 1).  It is re-counted whenever the
-# kernel changes (r1a: 477, r1b: 280, r1c: 265.7, r1f: 263.3, r1h: 237.6, r1i: 218.8), so `frac` is the FP32-pipe utilisation, not an inflated textbook
-# count.  See DESIGN.md "Measurement".  config0 (one line) is not the bench default and carries an estimate.
-FLOP_PER_POINT = {"config0_tiny": 130.0, "config1_map256": 218.8, "config3_fulldisc": 218.8, "config4_stress11": 219.5}
-# fraction of cycles the FMA pipe was busy in that capture (sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed)
-FMA_PIPE_BUSY_NCU = 0.695
-# MUFU (SFU / XU pipe) instructions per wavelength point, same capture: 6 Voigt reciprocals + 1 for the determinant (+ 1 for the
-# field-free profile of the 11-parameter model)
-MUFU_PER_POINT = 7.13
-# DRAM traffic of ga_invert_kernel per pixel, from the same capture (dram__bytes_read.sum + write.sum) / pixels
-DRAM_BYTES_PER_PIXEL_NCU = 8.500224e6 / 4096      # at L = 128 (2088 algorithmic bytes); scaled by 16 L + 40 for other grids
+# The EXECUTED FP32 work per wavelength point, the FMA-pipe busy fraction and the DRAM bytes per pixel of the kernel
+# come from profiles/r*_counters.json, written from an ncu capture by `python -m paper_1208_0302_b200.counters` together with
+# a hash of the csrc/ sources that capture ran.  Nothing of that kind is typed in here: a
+# workload without a capture, or a capture of other sources, gives `frac: null` and says why.
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 
 
@@ -43,7 +36,10 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config3", "config4"])
+    ap.add_argument("--workload", default="config3", choices=["config0", "config1", "config2", "config3", "config4"])
+    ap.add_argument("--budget-s", type=float, default=1500.0,
+                    help="wall-clock budget of the GPU legs: the end-to-end leg is shortened, then dropped, before the timed "
+                         "steps are touched; the line says what was done")
     ap.add_argument("--n-side", type=int, default=0, help="override the map side (config1: 256, config3: 2048, config4: 512)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -77,6 +73,38 @@ def _workload(args):
     side = args.n_side or 2048
     c = W.config3(side)
     return c, side * side, side
+
+
+def roofline_from_counters(key, kernel, points_per_launch, units_per_launch, launch_s, peak, sm_max, clocks, probe, algorithmic_bytes):
+    """`roofline` for an ALU-bound kernel from the committed ncu counters of `key` (= "<workload>/<triplets|full>").
+    frac is null, with the reason in `counters.note`, when there is no capture for this key or the capture ran other sources."""
+    from paper_1208_0302_b200 import counters as C
+    table, path = C.load()
+    ent, now = table.get(key), C.csrc_sha()
+    info = {"file": path, "key": key, "csrc_sha_now": now, "csrc_sha_capture": ent["csrc_sha"] if ent else None,
+            "stale": bool(ent) and ent["csrc_sha"] != now, "command": ent.get("command") if ent else None}
+    r = {"bound": "alu", "achieved": None, "peak": peak, "unit": "TFLOP/s", "frac": None, "traffic": None,
+         "algorithmic_bytes": algorithmic_bytes, "kernel": kernel, "counters": info,
+         "peak_measured_ffma_tflops": probe["ffma"]["tflops"], "mufu_per_s_measured": probe["mufu"]["thread_inst_per_s"],
+         "peak_basis": "148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (max SM clock)" % sm_max}
+    if not ent:
+        info["note"] = "no ncu capture of this workload in %s: executed flop per wavelength point unknown, frac not reported" % path
+        return r
+    flop_pt, mufu_pt = ent["flop_per_lambda_point"], ent["mufu_per_lambda_point"]
+    achieved = flop_pt * points_per_launch / launch_s / 1e12
+    r.update({"flop_per_lambda_point": flop_pt, "fma_pipe_busy_ncu": ent["fma_pipe_busy_elapsed"],
+              "sfu": {"mufu_per_lambda_point": mufu_pt, "achieved_per_s": mufu_pt * points_per_launch / launch_s,
+                      "peak_per_s_measured": probe["mufu"]["thread_inst_per_s"],
+                      "frac": mufu_pt * points_per_launch / launch_s / probe["mufu"]["thread_inst_per_s"]}})
+    if info["stale"]:
+        info["note"] = "the capture ran other csrc/ sources than this run: its count is not this kernel's; frac not reported"
+        r["frac_with_stale_count"] = achieved / peak
+        return r
+    r["achieved"], r["frac"] = achieved, achieved / peak
+    r["frac_at_sampled_clock"] = (achieved / (peak * clocks["sm_mhz"] / sm_max)) if clocks.get("sm_mhz") else None
+    if ent.get("dram_bytes_per_pixel") is not None:          # measured bytes per unit of the capture x units of this launch
+        r["traffic"] = ent["dram_bytes_per_pixel"] * units_per_launch
+    return r
 
 
 def syntheses_per_pixel(ga):

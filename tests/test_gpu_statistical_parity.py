@@ -118,7 +118,11 @@ def test_config1_statistical_parity(B):
     truth = W.draw_truth(n, seed=W.SEED_TRUTH, stream=11)
     ids, mu = np.arange(n), np.ones(n)
     out = invert_both(B, cfg, ids, truth, mu, noise_stream=11)
-    judge("config1", "config1: %d iid prior draws, two triplets, L = 128, pop 128, 100 generations" % n, truth, *out, min_same=0.9)
+    # The identical-optimum fraction is a diagnostic, not a north_star criterion: it measures how often the one binary32-vs-
+    # binary64 `<` (reading G4) parts two chaotic trajectories.  Measured on these 1024 pixels with the round-1 kernel:
+    # 90.3 % (sampling noise +- 0.9 %; 93.9 % with the more accurate r1f Voigt tiers).  Floor 0.85, fixed before any
+    # round-2 kernel change; a kernel that falls below it has lost accuracy and must say so, not move the floor.
+    judge("config1", "config1: %d iid prior draws, two triplets, L = 128, pop 128, 100 generations" % n, truth, *out, min_same=0.85)
 
 
 def test_config3_statistical_parity(B):
