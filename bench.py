@@ -44,7 +44,10 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-aux", action="store_true", help="skip the auxiliary me_synth (config2) measurement")
+    ap.add_argument("--aux", action="store_true", help="also run the auxiliary me_synth (config2) legs and saturation trace inside this run")
+    ap.add_argument("--no-aux", action="store_true", help="accepted for old command lines; the auxiliary legs are off unless --aux")
+    ap.add_argument("--vectors", type=int, default=1_000_000, help="config2: parameter vectors per step")
+    ap.add_argument("--chi2-only", action="store_true", help="config2: no [P,4,L] output, chi2 against the fixed profile only")
     ap.add_argument("--zeeman", default="triplets", choices=["triplets", "full"],
                     help="full = LS-coupling Zeeman patterns (12 + 3 components, PAPER.md:351) instead of effective triplets; "
                          "a measured variant, not the headline configuration")
@@ -59,6 +62,9 @@ def workload(args):
 
 
 def _workload(args):
+    if args.workload == "config2":
+        c = W.config2(args.vectors)
+        return c, args.vectors, None
     if args.workload == "config0":
         c = W.config0()
         return c, c["n_pixels"], None
@@ -170,16 +176,34 @@ def oracle_lines_for(cfg):
     return orc.Lines(lines, W.LAMBDA_REF)
 
 
+_FULLDISC = {}
+
+
 def oracle_sample(cfg, n, stream=0):
-    """n pixels of the workload, observations synthesised by the oracle itself (+ seeded noise, rounded to f32)."""
+    """n pixels of the workload, observations synthesised by the oracle itself (+ seeded noise, rounded to f32).
+    config3: pixels OF the full-disc map (80 % quiet / 20 % active region, mu per pixel) under their global ids.
+    Returns (lines, obs, nm_profile, mu or None, ids or None)."""
     from oracle import api as orc
     ln = oracle_lines_for(cfg)
     npar = cfg.get("npar", 9)
-    truth = W.draw_truth(n, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=100 + stream, npar=npar)
+    mu = ids = None
+    if "n_side" in cfg:
+        key = (cfg["n_side"], cfg["radius"])
+        if key not in _FULLDISC:
+            _FULLDISC[key] = W.fulldisc_truth(cfg["n_side"], cfg["radius"])
+        mask, mu_all, truth_all, active = _FULLDISC[key]
+        on = mask.astype(bool)
+        q, ac = np.flatnonzero(on & ~active), np.flatnonzero(on & active)
+        nq = n - n // 5
+        pick = lambda a, m: a[(stream * 7919 + np.arange(m) * max(1, a.size // max(m, 1))) % a.size]
+        ids = np.concatenate([pick(q, nq), pick(ac, n - nq)])
+        truth, mu = truth_all[ids], mu_all[ids]
+    else:
+        truth = W.draw_truth(n, seed=W.SEED_TRUTH, b_lo=cfg["b_range"][0], b_hi=cfg["b_range"][1], stream=100 + stream, npar=npar)
     nm = orc.synth(W.NM_PARAMS[None, :], cfg["lam"], ln)[0, 0] if npar == 11 else None
-    clean = orc.synth(truth, cfg["lam"], ln, threads=orc.hardware_threads(), nm_profile=nm)
+    clean = orc.synth(truth, cfg["lam"], ln, mu=mu, threads=orc.hardware_threads(), nm_profile=nm)
     obs = (clean + W.draw_noise(clean.shape, cfg["sigma"], stream=100 + stream)).astype(np.float32).astype(np.float64)
-    return ln, obs, nm
+    return ln, obs, nm, mu, ids
 
 
 def bounded_oracle_cfg(cfg, core_seconds_per_pixel=12.0):
@@ -200,10 +224,16 @@ def bounded_oracle_cfg(cfg, core_seconds_per_pixel=12.0):
 
 def time_oracle(cfg, n, stream=0):
     from oracle import api as orc
-    ln, obs, nm = oracle_sample(cfg, n, stream)
+    ln, obs, nm, mu, ids = oracle_sample(cfg, n, stream)
     cores = orc.hardware_threads()
     t0 = time.perf_counter()
-    orc.ga_invert(obs, cfg["lam"], ln, cfg["ga"], seed=W.SEED_GA, threads=cores, nm_profile=nm)
+    if ids is None:
+        orc.ga_invert(obs, cfg["lam"], ln, cfg["ga"], seed=W.SEED_GA, threads=cores, nm_profile=nm)
+    else:                                     # scattered global ids: one oracle call per pixel, spread over the cores
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(cores) as ex:         # ctypes releases the GIL
+            list(ex.map(lambda k: orc.ga_invert(obs[k:k + 1], cfg["lam"], ln, cfg["ga"], seed=W.SEED_GA, mu=mu[k:k + 1],
+                                                pixel_base=int(ids[k]), threads=1), range(n)))
     return time.perf_counter() - t0, cores
 
 
@@ -215,6 +245,23 @@ def run_reference(args):
     from oracle import api as orc
     cfg, n_pixels, _ = workload(args)
     cores = orc.hardware_threads()
+    if args.workload == "config2":            # the step is forward synthesis: the oracle's synth on a bounded batch per step
+        n, ln = 2000 * cores, oracle_lines_for(cfg)
+        t = 0.0
+        for k in range(args.warmup + args.steps):
+            truth = W.draw_truth(n, seed=W.SEED_TRUTH, stream=7 + k)
+            t0 = time.perf_counter(); orc.synth(truth, cfg["lam"], ln, threads=cores); dt = time.perf_counter() - t0
+            t += dt if k >= args.warmup else 0.0
+        val = n * args.steps / t
+        sample = "%d vectors of %s per step, all %d host threads" % (n, cfg["name"], cores)
+        print(json.dumps({"impl": "reference", "metric": "ME syntheses/s", "value": val, "unit": "syntheses/s", "n_gpus": args.gpus,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": cfg["name"], "vectors_per_step": n, "L": int(cfg["lam"].size), "lines": 2},
+                          "cpu_baseline": {"value": val, "unit": "syntheses/s", "cores": cores, "kind": "oracle", "sample": sample},
+                          "e2e": {"value": val, "unit": "syntheses/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0}), flush=True)
+        return
     ocfg, frac, note = bounded_oracle_cfg(cfg, core_seconds_per_pixel=6.0)
     per_pixel_points = syntheses_per_pixel(ocfg["ga"]) * cfg["lam"].size * sum(3 for _ in cfg["lines"])
     n = max(cores, int(cores * max(1.0, 2.0e7 / per_pixel_points)))      # ~ a few seconds of work per core per step
@@ -226,7 +273,8 @@ def run_reference(args):
         dt, _ = time_oracle(ocfg, n, stream=args.warmup + k)
         t += dt
     val = n * frac * args.steps / t
-    sample = "%d pixels of %s%s per step (oracle-synthesised obs), all %d host threads" % (n, cfg["name"], note, cores)
+    sample = "%d pixels of %s%s per step (%soracle-synthesised obs), all %d host threads" % (
+        n, cfg["name"], note, "map pixels stratified 80/20 quiet/active with their mu and global ids, " if "n_side" in cfg else "", cores)
     line = {"impl": "reference", "metric": "pixel-inversions/s", "value": val, "unit": "pixels/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -338,13 +386,39 @@ def run_b200(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    # Wall-clock budget (--budget-s): one step of config3 takes about a minute, and the driver asks for 5 + 20 of them.
+    # The first warm-up step is timed on the host; if warm-up + K steps + the end-to-end leg would not fit, the end-to-end
+    # leg is cut to one step without its own warm-up, then dropped; K is reduced only if the steps alone do not fit, and
+    # the line then carries the K that was timed and says so.
+    t_wall0 = time.perf_counter()
+    notes = []
+    steps = args.steps
+    t_step = None
+    for w in range(args.warmup):
+        t0 = time.perf_counter()
         step()
+        if w == 0:
+            torch.cuda.synchronize()
+            t_step = time.perf_counter() - t0
     barrier()
+    if t_step is None:
+        t0 = time.perf_counter(); step(); torch.cuda.synchronize(); t_step = time.perf_counter() - t0
+        notes.append("warmup 0 requested: one untimed step was run to size the budget")
+    left = args.budget_s - (time.perf_counter() - t_wall0)
+    e2e_plan = 0 if args.no_e2e else (3 if t_step < 20.0 else 1)          # e2e steps incl. its warm-up (none when a step is long)
+    if not args.no_e2e and (steps + e2e_plan) * t_step > left:
+        e2e_plan = 1 if (steps + 1) * t_step <= left else 0
+        notes.append("end-to-end leg %s to fit --budget-s %.0f" % ("cut to one step" if e2e_plan else "dropped", args.budget_s))
+    if steps * t_step > left:
+        steps = max(1, int(left / t_step))
+        notes.append("TIMED %d OF THE %d STEPS ASKED FOR: %d x %.1f s does not fit --budget-s %.0f" % (steps, args.steps, args.steps, t_step, args.budget_s))
+    if world > 1:                                                          # every rank must run the same plan
+        plan = torch.tensor([steps, e2e_plan], device="cuda"); dist.all_reduce(plan, op=dist.ReduceOp.MIN)
+        steps, e2e_plan = int(plan[0].item()), int(plan[1].item())
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clk:
         ev0.record()
-        for _ in range(args.steps):
+        for _ in range(steps):
             step()
         ev1.record()
         barrier()
@@ -355,7 +429,7 @@ def run_b200(args):
 
     # end to end through the C ABI from HOST buffers: pinned obs -> H2D -> ga_invert -> D2H of params + chi2
     e2e = None
-    if not args.no_e2e:
+    if e2e_plan > 0:
         h_obs = torch.empty(obs.shape, dtype=torch.float32, pin_memory=True); h_obs.copy_(obs)
         h_p = torch.empty(out_p.shape, dtype=torch.float32, pin_memory=True)
         h_c = torch.empty(out_c.shape, dtype=torch.float32, pin_memory=True)
@@ -368,9 +442,11 @@ def run_b200(args):
             B.ga_invert(d_obs, lam, ld, ga, W.SEED_GA, mask=mask_t, mu=mu_t, pixel_id_base=base, out_params=out_p, out_chi2=out_c)
             h_p.copy_(out_p, non_blocking=True); h_c.copy_(out_c, non_blocking=True)
 
-        e2e_step(); barrier()
+        if e2e_plan > 1:
+            e2e_step()                                   # its own warm-up (the kernel itself is warm either way)
+        barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        n_e2e = max(1, min(args.steps, 2))
+        n_e2e = max(1, min(steps, e2e_plan - 1)) if e2e_plan > 1 else 1
         e0.record()
         for _ in range(n_e2e):
             e2e_step()
@@ -386,13 +462,11 @@ def run_b200(args):
         return
 
     sec = ms * 1e-3
-    value = world * n_active * args.steps / sec
+    value = world * n_active * steps / sec
     syn = syntheses_per_pixel(ga)
     L = int(lam.size)
     points_per_launch = n_active * syn * L
-    flop_pt = FLOP_PER_POINT[cfg["name"]]
-    launch_s = sec / args.steps
-    achieved = flop_pt * points_per_launch / launch_s / 1e12
+    launch_s = sec / steps
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -402,28 +476,25 @@ def run_b200(args):
     peak = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     clocks = clk.summary()
     # the FP32 FMA rate this box actually sustains (scalar FFMA probe of the library, 8 resident CTAs/SM), for context
-    from paper_1208_0302_b200 import peaks as mepeaks
+    from paper_1208_0302_b200 import peaks as mepeaks, counters as mecounters
     probe = mepeaks.measure(iters=2048, kinds=(0, 3))["probes"]
-    line = {"metric": "pixel-inversions/s", "value": value, "unit": "pixels/s", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+    key = "%s/%s" % (cfg["name"], "triplets" if cfg["triplets"] else "full")
+    roof = roofline_from_counters(key, "ga_invert_kernel", points_per_launch, n_active, launch_s, peak, sm_max, clocks, probe,
+                                  (16 * L + 40) * n_active)
+    line = {"metric": "pixel-inversions/s", "value": value, "unit": "pixels/s", "n_gpus": world, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg["name"], "pixels_per_gpu": n_pixels, "active_pixels_per_gpu": n_active, "L": L,
                        "pop": ga["pop"], "generations": ga["generations"], "lines": len(cfg["lines"]),
                        "zeeman": "effective triplets" if cfg["triplets"] else "full LS patterns", "parallelism": "pixel shards x%d" % world,
                        "l2": "obs cube %.0f MB per step (> 126 MB L2 for config1/3); path is ALU-bound" % (obs.numel() * 4 / 1e6)},
-            "syntheses_per_s": value * syn, "median_chi2": med_chi2,
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": DRAM_BYTES_PER_PIXEL_NCU * n_active * (16 * L + 40) / 2088.0, "algorithmic_bytes": (16 * L + 40) * n_active,
-                         "kernel": "ga_invert_kernel", "flop_per_lambda_point": flop_pt, "fma_pipe_busy_ncu": FMA_PIPE_BUSY_NCU,
-                         "peak_measured_ffma_tflops": probe["ffma"]["tflops"],
-                         "mufu_per_s_measured": probe["mufu"]["thread_inst_per_s"],
-                         "sfu": {"mufu_per_lambda_point": MUFU_PER_POINT, "achieved_per_s": MUFU_PER_POINT * points_per_launch / launch_s,
-                                 "peak_per_s_measured": probe["mufu"]["thread_inst_per_s"],
-                                 "frac": MUFU_PER_POINT * points_per_launch / launch_s / probe["mufu"]["thread_inst_per_s"]},
-                         "peak_basis": "148 SM x 128 FP32 lanes x 2 flop x %.0f MHz (max SM clock)" % sm_max,
-                         "frac_at_sampled_clock": (achieved / (peak * clocks["sm_mhz"] / sm_max)) if clocks.get("sm_mhz") else None},
-            "clocks": clocks, "gpu_launches": args.steps, "e2e": e2e}
-    if not args.no_aux:
+            "syntheses_per_s": value * syn, "median_chi2": med_chi2, "roofline": roof,
+            "clocks": clocks, "gpu_launches": steps, "e2e": e2e, "csrc_sha": mecounters.csrc_sha()}
+    if steps != args.steps:
+        line["steps_requested"] = args.steps
+    if notes:
+        line["notes"] = notes
+    if args.aux:
         line["me_synth_config2"] = bench_me_synth(torch, B, peaks)
         # BASELINE config 2's saturation trace: P = 1e4 .. 1e7 with the full [P,4,L] output (20.5 GB at 1e7)
         line["me_synth_config2"]["saturation"] = {
@@ -434,7 +505,7 @@ def run_b200(args):
         from oracle import api as orc
         cores = orc.hardware_threads()
         ocfg, frac, note = bounded_oracle_cfg(cfg)
-        n = min(n_pixels, (2 if frac == 1.0 else 1) * cores)
+        n = min(n_pixels, (4 if frac == 1.0 else 1) * cores)        # ~10-30 s on the box's cores; BASELINE.md says why not more
         dt, cores = time_oracle(ocfg, n)
         line["cpu_baseline"] = {"value": n * frac / dt, "unit": "pixels/s", "cores": cores, "kind": "oracle",
                                 "sample": "%d pixels of %s%s, oracle-synthesised obs, %.1f s" % (n, cfg["name"], note, dt)}
@@ -443,9 +514,105 @@ def run_b200(args):
         dist.destroy_process_group()
 
 
+def run_config2(args):
+    """BASELINE config 2 as the step: me_synth over `--vectors` iid prior draws on the two-line 128-point grid, [P,4,L] output
+    + chi2 against one fixed profile (or --chi2-only).  Single GPU; the ordering workspace is allocated ONCE by the caller
+    (me_synth_ws), so the timed region holds the library's launches only."""
+    import torch
+    from paper_1208_0302_b200 import binding as B, build as mebuild, peaks as mepeaks, counters as mecounters
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    mebuild.build(); B.lib()
+    P = args.vectors
+    c2 = W.config2(P)
+    lam, ld, L = c2["lam"], B.line_data_from_workload(c2["lines"], True), int(c2["lam"].size)
+    params = torch.from_numpy(W.draw_truth(P, seed=W.SEED_TRUTH, stream=7).astype(np.float32)).cuda()
+    obs_ref = B.me_synth(params[:1].contiguous(), lam, ld)[0][0].contiguous()
+    wos = c2["ga"]["stokes_weight"] / c2["ga"]["sigma"]
+    out = None if args.chi2_only else torch.empty((P, 4, L), dtype=torch.float32, device="cuda")
+    chi = torch.empty((P,), dtype=torch.float32, device="cuda")
+    need = B.me_synth_workspace_bytes(P)
+    ws = torch.empty((need,), dtype=torch.uint8, device="cuda") if need else False
+
+    def step():
+        B.me_synth(params, lam, ld, out_stokes=out, obs_ref=obs_ref, w_over_sigma=wos, out_chi2=chi, want_stokes=not args.chi2_only, workspace=ws)
+
+    for _ in range(max(args.warmup, 1)):
+        step()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(0) as clk:
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+        ev1.record()
+        torch.cuda.synchronize()
+    sec = ev0.elapsed_time(ev1) * 1e-3
+    launch_s = sec / args.steps
+    e2e = None
+    if not args.no_e2e:                      # host params -> H2D -> me_synth -> D2H of chi2 (and of the cube when it is produced)
+        h_p = torch.empty(params.shape, dtype=torch.float32, pin_memory=True); h_p.copy_(params)
+        h_c = torch.empty(chi.shape, dtype=torch.float32, pin_memory=True)
+        h_o = None if out is None else torch.empty(out.shape, dtype=torch.float32, pin_memory=True)
+        d_p = torch.empty_like(params)
+
+        def e2e_step():
+            d_p.copy_(h_p, non_blocking=True)
+            B.me_synth(d_p, lam, ld, out_stokes=out, obs_ref=obs_ref, w_over_sigma=wos, out_chi2=chi, want_stokes=not args.chi2_only, workspace=ws)
+            h_c.copy_(chi, non_blocking=True)
+            if h_o is not None:
+                h_o.copy_(out, non_blocking=True)
+        e2e_step(); torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            e2e_step()
+        e1.record(); torch.cuda.synchronize()
+        e2e = {"value": P * args.steps / (e0.elapsed_time(e1) * 1e-3), "unit": "syntheses/s", "h2d_bytes_per_step": h_p.numel() * 4,
+               "d2h_bytes_per_step": (h_c.numel() + (h_o.numel() if h_o is not None else 0)) * 4, "steps": args.steps}
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    clocks = clk.summary()
+    probe = mepeaks.measure(iters=2048, kinds=(0, 3))["probes"]
+    nbytes = P * (36 + 4 + (0 if args.chi2_only else 16 * L))
+    key = "config2_synth_sweep/%s" % ("chi2_only" if args.chi2_only else "stokes")
+    roof = roofline_from_counters(key, "me_synth_kernel", P * L, P, launch_s, peak, sm_max, clocks, probe, nbytes)
+    roof["hbm"] = {"achieved_gbs": nbytes / launch_s / 1e9, "peak_gbs_measured": float(peaks.get("hbm_gbs", 0.0)) or None,
+                   "frac": (nbytes / launch_s / 1e9 / float(peaks["hbm_gbs"])) if peaks.get("hbm_gbs") else None}
+    n_launch = (4 if need else 1)
+    line = {"metric": "ME syntheses/s", "value": P / launch_s, "unit": "syntheses/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 1), "ms_per_step": launch_s * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": c2["name"], "vectors": P, "L": L, "lines": 2, "zeeman": "effective triplets",
+                       "output": "chi2 only" if args.chi2_only else "[P,4,L] Stokes + chi2",
+                       "l2": "output %.0f MB per step (> 126 MB L2)" % (nbytes / 1e6) if not args.chi2_only else "inputs 40 MB per step; path is ALU-bound",
+                       "ordered_visit": bool(need)},
+            "roofline": roof, "clocks": clocks, "gpu_launches": args.steps * n_launch, "e2e": e2e, "csrc_sha": mecounters.csrc_sha()}
+    if not args.no_cpu_baseline:
+        from oracle import api as orc
+        cores = orc.hardware_threads()
+        n = 2000 * cores
+        truth = W.draw_truth(n, seed=W.SEED_TRUTH, stream=7)
+        ln = oracle_lines_for(c2)
+        t0 = time.perf_counter(); orc.synth(truth, lam, ln, threads=cores); dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": n / dt, "unit": "syntheses/s", "cores": cores, "kind": "oracle",
+                                "sample": "%d vectors of %s, %.1f s" % (n, c2["name"], dt)}
+    print(json.dumps(line), flush=True)
+
+
 if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.workload == "config2":
+        run_config2(a)
     else:
         run_b200(a)
