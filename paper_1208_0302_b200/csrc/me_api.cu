@@ -25,6 +25,11 @@ int build_synth_desc(const double* lambda, int L, const me_line_data* ld, me::Sy
     if (L < 2 || L > ME_MAX_L) return ME_ERR_SHAPE;
     if (ld->n_lines < 1 || ld->n_lines > ME_MAX_LINES) return ME_ERR_SHAPE;
     if (ld->n_params != ME_NPAR && ld->n_params != ME_MAX_NPAR) return ME_ERR_SHAPE;
+    if (4 * L <= ld->n_params) return ME_ERR_SHAPE;           // nu = 4 L - M of eq. 16 must be positive
+    for (int j = 0; j < L; ++j) {                             // finite and strictly increasing (the prologue's lobe order and
+        if (!std::isfinite(lambda[j])) return ME_ERR_RANGE;   // centre of gravity, readings P1 / S1, assume ascending wavelength)
+        if (j > 0 && !(lambda[j] > lambda[j - 1])) return ME_ERR_RANGE;
+    }
     if (ld->n_params == ME_MAX_NPAR && ld->nm_profile == nullptr) return ME_ERR_NULL;   // reading F13 needs I_fixed
     if (ld->n_params == ME_NPAR && ld->nm_profile != nullptr) return ME_ERR_SHAPE;
     if (!(ld->lambda_ref_A > 0.0)) return ME_ERR_RANGE;
@@ -87,23 +92,29 @@ void sobol_directions16(int dim, uint32_t v[16]) {
     for (int i = 1; i <= 16; ++i) v[i - 1] = m[i] << (32 - i);
 }
 
+// box_only: the caller is ga_uncertainty or ga_prologue, for which me.h says "the GA fields of cfg are ignored": population,
+// generations, tournament, elitism, probabilities and the mutation schedule are neither checked nor used.
 int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t seed, int64_t N, bool need_sigma,
-                  me::GaDesc& g) {
+                  me::GaDesc& g, bool box_only = false) {
     if (c == nullptr) return ME_ERR_NULL;
     if (npar != ME_NPAR && npar != ME_MAX_NPAR) return ME_ERR_SHAPE;
     if (need_sigma && sigma == nullptr) return ME_ERR_NULL;
-    if (c->pop < 2 || c->pop > ME_MAX_POP) return ME_ERR_SHAPE;
-    if (c->generations < 0 || c->generations > ME_MAX_GEN) return ME_ERR_SHAPE;
-    if (c->tournament_k < 1 || c->tournament_k > 4) return ME_ERR_RANGE;
-    if (c->elite != 1) return ME_ERR_UNSUPPORTED;
+    if (!box_only) {
+        if (c->pop < 2 || c->pop > ME_MAX_POP) return ME_ERR_SHAPE;
+        if (c->generations < 0 || c->generations > ME_MAX_GEN) return ME_ERR_SHAPE;
+        if (c->tournament_k < 1 || c->tournament_k > 4) return ME_ERR_RANGE;
+        if (c->elite != 1) return ME_ERR_UNSUPPORTED;
+        if (!(c->p_cross >= 0.f && c->p_cross <= 1.f) || !(c->p_mut >= 0.f && c->p_mut <= 1.f)) return ME_ERR_RANGE;
+        if ((c->prologue & 4) && c->pop < 3) return ME_ERR_SHAPE;             // reading S1: the seeds take the last two slots of P0
+    }
     if (c->variant != 0 && c->variant != 1) return ME_ERR_RANGE;
     if (c->prologue < 0 || c->prologue > 7) return ME_ERR_RANGE;
     if ((c->prologue & 2) && c->log_scale[1]) return ME_ERR_UNSUPPORTED;      // the polarity box is linear in gamma
-    if (!(c->p_cross >= 0.f && c->p_cross <= 1.f) || !(c->p_mut >= 0.f && c->p_mut <= 1.f)) return ME_ERR_RANGE;
     if (c->pixel_id_base < 0 || N < 0 || (uint64_t)c->pixel_id_base + (uint64_t)N > 0x100000000ULL) return ME_ERR_RANGE;
     std::memset(&g, 0, sizeof(g));
     g.pop = c->pop; g.generations = c->generations; g.tournament_k = c->tournament_k;
     g.p_cross = c->p_cross; g.p_mut = c->p_mut;
+    if (box_only) { g.pop = 3; g.generations = 0; g.tournament_k = 1; g.p_cross = g.p_mut = 0.f; }
     g.key0 = (uint32_t)(seed & 0xffffffffu); g.key1 = (uint32_t)(seed >> 32);
     g.pixel_base = (uint32_t)c->pixel_id_base;
     g.inv_nu = (float)(1.0 / (4.0 * L - npar));          // nu = 4 N_lambda - M
@@ -130,7 +141,7 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
     g.variant = c->variant;
     g.n_samp = c->generations / 4 > 1 ? c->generations / 4 : 1;
     for (int j = 0; j < ME_MAX_NPAR; ++j) sobol_directions16(j, g.sobol_v[j]);
-    if (c->variant == 1) return ME_OK;                        // the mutation-scale schedule is not used
+    if (c->variant == 1 || box_only) return ME_OK;            // the mutation-scale schedule is not used
     if (c->mut_scale_table != nullptr) {
         for (int t = 0; t <= c->generations; ++t) g.mut_scale[t] = c->mut_scale_table[t];
     } else {
@@ -234,7 +245,7 @@ int ga_uncertainty(const float* obs, int64_t N, const uint8_t* mask, const float
     me::SynthDesc sd; me::GaDesc gd;
     int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
     if (rc != ME_OK) return rc;
-    rc = build_ga_desc(cfg, sd.npar, sigma, L, 0, N, true, gd);
+    rc = build_ga_desc(cfg, sd.npar, sigma, L, 0, N, true, gd, true);
     if (rc != ME_OK) return rc;
     if (N == 0) return ME_OK;
     if (obs == nullptr || params == nullptr || out_sigma == nullptr) return ME_ERR_NULL;
@@ -272,7 +283,7 @@ int ga_prologue(const float* obs, int64_t N, const float* sigma, const double* l
     me::SynthDesc sd; me::GaDesc gd;
     int rc = build_synth_desc(lambda_grid_A, L, line_data, sd);
     if (rc != ME_OK) return rc;
-    rc = build_ga_desc(cfg, sd.npar, sigma, L, 0, N, true, gd);
+    rc = build_ga_desc(cfg, sd.npar, sigma, L, 0, N, true, gd, true);
     if (rc != ME_OK) return rc;
     fill_seed_desc(line_data, gd);
     if (N == 0) return ME_OK;

@@ -252,6 +252,11 @@ cudaError_t launch_ga_step(const GaDesc& gd, int npar, const float* genes_in, co
                            float* genes_out, cudaStream_t st) {
     const int threads = ((gd.pop + 31) / 32) * 32;
     const size_t smem = (size_t)gd.pop * npar * 4 + (size_t)gd.pop * 4 + 64 * 4 + (size_t)2 * gd.pop + 16;
+    // pop = 1024 with 11 genes needs 51 472 B: above the 48 KB a kernel gets without opting in (me.h allows pop up to ME_MAX_POP)
+    cudaError_t e = npar == ME_MAX_NPAR
+        ? cudaFuncSetAttribute(ga_step_kernel<ME_MAX_NPAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+        : cudaFuncSetAttribute(ga_step_kernel<ME_NPAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     if (npar == ME_MAX_NPAR) ga_step_kernel<ME_MAX_NPAR><<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
     else ga_step_kernel<ME_NPAR><<<grid_for(N), threads, smem, st>>>(gd, genes_in, chi2_in, N, t, genes_out);
     return cudaGetLastError();

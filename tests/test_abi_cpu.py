@@ -103,6 +103,25 @@ def test_argument_validation_without_gpu(lib):
     assert call(ld=ld11.c) == -2
     ld9 = B.line_data_from_workload(c0["lines"], True); ld9.c.nm_profile = 16
     assert call(ld=ld9.c) == -2                                # a fixed profile makes no sense with 9 parameters
+    # nu = 4 L - M of eq. 16 must be positive: L = 2 gives 8 - 9 < 0 (the argmin compares raw float bits, a negative chi2 breaks it)
+    assert call(L=2) == -2
+    # the wavelength grid must be finite and strictly increasing (lobe order and centre of gravity of the prologue assume it)
+    for bad_lam in (lam[::-1].copy(), np.where(np.arange(lam.size) == 7, np.nan, lam), np.where(np.arange(lam.size) == 7, lam[6], lam)):
+        assert call(lam=np.ascontiguousarray(bad_lam).ctypes.data_as(C.POINTER(C.c_double))) == -3
+    # reading S1: the seeds take the last two slots of P0, a population of 2 has no room for them
+    bad = B._GaCfg.from_buffer_copy(cfg); bad.prologue = 4; bad.pop = 2
+    assert call(cfg=bad) == -2
+    bad.pop = 3
+    assert call(cfg=bad, N=0) == 0
+    # ga_uncertainty and ga_prologue ignore the GA fields of cfg (me.h): garbage there is not an error for them ...
+    junk = B._GaCfg.from_buffer_copy(cfg)
+    junk.pop, junk.generations, junk.tournament_k, junk.elite, junk.p_cross, junk.p_mut = 0, -5, 99, 0, 7.0, -1.0
+    junk.mut_scale_table = C.POINTER(C.c_float)(); junk.mut_scale0 = junk.mut_scale_end = 0.0
+    assert call(cfg=junk) != 0                                 # ... while ga_invert refuses it
+    assert lib.ga_uncertainty(one, C.c_int64(0), None, sig, lam_p, C.c_int(lam.size), C.byref(ld.c), C.byref(junk), one, one, one, None) == 0
+    assert lib.ga_prologue(one, C.c_int64(0), sig, lam_p, C.c_int(lam.size), C.byref(ld.c), C.byref(junk), one, None) == 0
+    junk.lo[3] = 60.0                                          # their box checks stay
+    assert lib.ga_uncertainty(one, C.c_int64(0), None, sig, lam_p, C.c_int(lam.size), C.byref(ld.c), C.byref(junk), one, one, one, None) == -3
     # me_synth
     assert lib.me_synth(one, C.c_int64(0), None, lam_p, C.c_int(lam.size), C.byref(ld.c), one, None, None, None, None) == 0
     assert lib.me_synth(one, C.c_int64(5), None, lam_p, C.c_int(lam.size), C.byref(ld.c), None, None, None, None, None) == -1

@@ -65,7 +65,8 @@ def test_me_synth11_vs_oracle(B, name, lines, triplets, lam, P):
     assert np.max(np.abs(chi.cpu().numpy() - want) / want) < 2e-4
 
 
-@pytest.mark.parametrize("pop,k", [(64, 3), (100, 2), (512, 3)])
+# pop = 1024 with 11 genes: ga_step's 51 472 B of dynamic shared memory need the > 48 KB opt-in (ME_MAX_POP, me.h)
+@pytest.mark.parametrize("pop,k", [(64, 3), (100, 2), (512, 3), (1024, 3)])
 def test_ga_init_and_step_bit_exact_eleven_genes(B, pop, k):
     cfg = W.ga_config(pop, 12, tournament_k=k, npar=11)
     N, seed, base = 19, 0x5EED5EED5, 123456
