@@ -150,6 +150,20 @@ def seeds(obs, lam, lines, cfg):
     return out
 
 
+def seed_auer(obs, lam, lines, cfg, glo=None, ghi=None):
+    """Reading S2: obs[N,4,L] -> [N,7] = B_los [G], gamma, chi [deg], B [G], and the 10-bit box coordinates (q_B, q_gamma, q_chi)
+    of the Auer weak-field member; glo/ghi[N] = per-pixel inclination box (default: the configured one)."""
+    obs, lam = _f64(obs), _f64(lam)
+    N, L = obs.shape[0], lam.size
+    glo = np.full(N, float(cfg["lo"][1])) if glo is None else _f64(glo)
+    ghi = np.full(N, float(cfg["hi"][1])) if ghi is None else _f64(ghi)
+    out = np.empty((N, 7))
+    lib().orc_seed_auer(_p(obs, C.c_double), C.c_int64(N), _p(lam, C.c_double), C.c_int(L), *lines.args(),
+                        C.c_double(cfg["lo"][0]), C.c_double(cfg["hi"][0]), C.c_int(int(cfg["log_scale"][0])),
+                        C.c_double(cfg["lo"][2]), C.c_double(cfg["hi"][2]), _p(glo, C.c_double), _p(ghi, C.c_double), _p(out, C.c_double))
+    return out
+
+
 def sobol(n0, count, dims):
     out = np.zeros((count, dims), dtype=np.uint32)
     lib().orc_sobol(C.c_uint32(n0), C.c_int(count), C.c_int(dims), _p(out, C.c_uint32))

@@ -140,6 +140,18 @@ void orc_seeds(const double* obs, int64_t N, const double* lambda, int L,
     for (int64_t n = 0; n < N; ++n) pixel_seeds(obs + n * 4 * L, lambda, L, ln, c, out + n * 3);
 }
 
+// Auer weak-field member of one batch (reading S2): obs[N][4][L] -> out[N][7] = B_los, gamma, chi, B, q_B, q_gamma, q_chi.
+// glo/ghi[N]: the per-pixel inclination box (the configured one, or the polarity-cut one of reading P1).
+void orc_seed_auer(const double* obs, int64_t N, const double* lambda, int L,
+                   int n_lines, const double* lambda0, const double* strength, const int* n_comp,
+                   const double* shift, const double* weight, const int* kind, double lambda_ref,
+                   double b_lo, double b_hi, int b_log, double chi_lo, double chi_hi, const double* glo, const double* ghi,
+                   double* out) {
+    Lines ln = make_lines(n_lines, lambda0, strength, n_comp, shift, weight, kind, lambda_ref);
+    GaCfg c; c.lo[P_B] = b_lo; c.hi[P_B] = b_hi; c.log_scale[P_B] = b_log; c.lo[P_CHI] = chi_lo; c.hi[P_CHI] = chi_hi;
+    for (int64_t n = 0; n < N; ++n) pixel_seed_auer(obs + n * 4 * L, lambda, L, ln, c, glo[n], ghi[n], out + n * 7);
+}
+
 // count Sobol' points starting at index n0, dims dimensions: out[count][dims] (32-bit fixed point).
 void orc_sobol(uint32_t n0, int count, int dims, uint32_t* out) {
     for (int i = 0; i < count; ++i)

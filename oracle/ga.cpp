@@ -258,6 +258,97 @@ void pixel_seeds(const double* obs, const double* lambda, int L, const Lines& ln
     out[2] = blos >= 0.0 ? 0.0 : 1023.0;
 }
 
+// Reading S2: the weak-field member of P0 "as in Auer et al. (1977)".  The paper states its content in two places:
+// "the longitudinal field strength is calculated from the separation between the I+-V line-cores, while the field orientation
+// is calculated from Stokes Q, U, and V maxima" and "the seed fields are checked to ensure that they are
+// consistent with this polarity".  Weak-field theory (Zeeman splitting dl_B = C g lambda0^2 B << Doppler width):
+//   V = -dl_B cos(gamma) I',    (Q, U) = -(1/4) dl_B^2 sin^2(gamma) I'' (cos 2chi, sin 2chi).
+// On the seed line's window of reading S1 (samples with |lambda - lambda0| <= hw; "interior" = both neighbours inside too):
+//   1. core of y = I+V and of y = I-V: first minimum sample, refined by the vertex of the parabola through it and its two
+//      neighbours when it is interior;  B_los = (lambda_+ - lambda_-) / (2 C g lambda0^2)   (I+V sees sigma_red, pin P2)
+//   2. I', I'' by three-point differences on the interior samples; D1 = max |I'|, D2 = max |I''|, Vm = max |V|,
+//      jL = first maximum of Q^2 + U^2, Lm = sqrt of it
+//   3. chi = (1/2) atan2(s U_jL, s Q_jL) mod 180 deg with s = -1 where I'' >= 0 at jL (line core), +1 otherwise
+//   4. tan(gamma') = 2 sqrt(Lm) D1 / (Vm sqrt(D2)), gamma' in [0, 90] (90 when Vm = 0 or D2 = 0);
+//      gamma = gamma' for B_los >= 0, else 180 - gamma'; if that lies outside the pixel's inclination box [glo, ghi]
+//      (polarity restriction, reading P1) it is reflected, gamma -> 180 - gamma, then clamped to the box
+//   5. B = |B_los| / max(|cos gamma|, 1/8), clamped to its box
+// out: [0] B_los (G), [1] gamma (deg), [2] chi (deg), [3] B (G), [4..6] the 10-bit box coordinates q of (B, gamma, chi).
+void pixel_seed_auer(const double* obs, const double* lambda, int L, const Lines& ln, const GaCfg& c, double glo, double ghi,
+                     double out[7]) {
+    const double CZ = 4.66857e-13;
+    int best = 0; double gbest = -1.0, sens = -1.0;
+    for (size_t l = 0; l < ln.lines.size(); ++l) {
+        double g = 0.0;
+        for (const Component& k : ln.lines[l].comps) if (k.kind == 1) g += k.weight * k.shift;
+        const double s = g * ln.lines[l].lambda0 * ln.lines[l].lambda0;
+        if (s > sens) { sens = s; best = (int)l; gbest = g; }
+    }
+    const double l0 = ln.lines[best].lambda0;
+    double hw = std::numeric_limits<double>::infinity();
+    for (size_t l = 0; l < ln.lines.size(); ++l)
+        if ((int)l != best) hw = std::fmin(hw, 0.5 * std::fabs(ln.lines[l].lambda0 - l0));
+    const double *I = obs, *Q = obs + L, *U = obs + 2 * L, *V = obs + 3 * L;
+    auto in = [&](int j) { return j >= 0 && j < L && std::fabs(lambda[j] - l0) <= hw; };
+    auto interior = [&](int j) { return in(j - 1) && in(j) && in(j + 1); };
+    // 1. line cores of I + V and I - V
+    double core[2] = { 0.0, 0.0 };
+    for (int k = 0; k < 2; ++k) {
+        const double sg = k == 0 ? 1.0 : -1.0;
+        int jm = -1; double ym = 0.0;
+        for (int j = 0; j < L; ++j) {
+            if (!in(j)) continue;
+            const double y = I[j] + sg * V[j];
+            if (jm < 0 || y < ym) { jm = j; ym = y; }
+        }
+        if (jm < 0) { for (int q = 0; q < 7; ++q) out[q] = 0.0; return; }
+        double x = lambda[jm] - l0;
+        if (interior(jm)) {
+            const double x0 = lambda[jm - 1] - l0, x2 = lambda[jm + 1] - l0;
+            const double y0 = I[jm - 1] + sg * V[jm - 1], y2 = I[jm + 1] + sg * V[jm + 1];
+            const double a0 = x - x0, a2 = x - x2, num = a0 * a0 * (ym - y2) - a2 * a2 * (ym - y0), den = a0 * (ym - y2) - a2 * (ym - y0);
+            if (den != 0.0) x -= 0.5 * num / den;
+        }
+        core[k] = x;
+    }
+    const double blos = gbest > 0.0 ? (core[0] - core[1]) / (2.0 * CZ * gbest * l0 * l0) : 0.0;
+    // 2. derivative measures of I and the polarisation maxima, interior samples
+    double D1 = 0.0, D2 = 0.0, Vm = 0.0, L2m = -1.0, d2L = 0.0, QL = 0.0, UL = 0.0;
+    for (int j = 0; j < L; ++j) {
+        if (!interior(j)) continue;
+        const double hm = lambda[j] - lambda[j - 1], hp = lambda[j + 1] - lambda[j];
+        const double d1 = (I[j + 1] - I[j - 1]) / (hm + hp);
+        const double d2 = 2.0 * ((I[j + 1] - I[j]) / hp - (I[j] - I[j - 1]) / hm) / (hm + hp);
+        D1 = std::fmax(D1, std::fabs(d1)); D2 = std::fmax(D2, std::fabs(d2)); Vm = std::fmax(Vm, std::fabs(V[j]));
+        const double l2 = Q[j] * Q[j] + U[j] * U[j];
+        if (l2 > L2m) { L2m = l2; d2L = d2; QL = Q[j]; UL = U[j]; }
+    }
+    if (L2m < 0.0) L2m = 0.0;
+    // 3. azimuth
+    const double s = d2L >= 0.0 ? -1.0 : 1.0;
+    double chi = 0.5 * std::atan2(s * UL, s * QL) * 180.0 / M_PI;
+    if (chi < 0.0) chi += 180.0;
+    if (chi >= 180.0) chi -= 180.0;
+    // 4. inclination
+    double gp = 90.0;
+    if (Vm > 0.0 && D2 > 0.0) gp = std::atan(2.0 * std::sqrt(std::sqrt(L2m)) * D1 / (Vm * std::sqrt(D2))) * 180.0 / M_PI;
+    double gam = blos >= 0.0 ? gp : 180.0 - gp;
+    if (gam < glo || gam > ghi) gam = 180.0 - gam;
+    gam = std::fmin(std::fmax(gam, glo), ghi);
+    // 5. field strength
+    const double cg = std::fmax(std::fabs(std::cos(gam * M_PI / 180.0)), 0.125);
+    const double b = std::fmin(std::fmax(std::fabs(blos) / cg, c.lo[P_B]), c.hi[P_B]);
+    auto coord = [&](double v, double lo, double hi, int logs) {
+        if (!(hi > lo)) return 0.0;
+        const double u = logs ? std::log(v / lo) / std::log(hi / lo) : (v - lo) / (hi - lo);
+        return std::rint(std::fmin(std::fmax(u, 0.0), 1.0) * 1023.0);
+    };
+    out[0] = blos; out[1] = gam; out[2] = chi; out[3] = b;
+    out[4] = coord(b, c.lo[P_B], c.hi[P_B], c.log_scale[P_B]);
+    out[5] = coord(gam, glo, ghi, 0);
+    out[6] = coord(std::fmin(std::fmax(chi, c.lo[P_CHI]), c.hi[P_CHI]), c.lo[P_CHI], c.hi[P_CHI], 0);
+}
+
 // stored gene for a 10-bit box coordinate q: the real-coded variant holds q / 1023 (one binary32 division), the
 // binary-coded variant the 16-bit code q << 6
 static float seed_gene(double q, const GaCfg& c) { return c.variant == 1 ? (float)(64.0 * q) : (float)q / 1023.0f; }
@@ -281,6 +372,13 @@ void ga_invert_pixel(const double* obs, double mu, const double* lambda, int L, 
         genes[(c.pop - 1) * M + P_B] = seed_gene(0.0, c);
         genes[(c.pop - 2) * M + P_B] = seed_gene(sd[1], c);
         genes[(c.pop - 2) * M + P_GAMMA] = seed_gene(sd[2], c);
+    }
+    if ((c0.prologue & 8) && c.pop >= 4) {                          // reading S2: the Auer weak-field member, slot P-3
+        double au[7];
+        pixel_seed_auer(obs, lambda, L, ln, c, c.lo[P_GAMMA], c.hi[P_GAMMA], au);
+        genes[(c.pop - 3) * M + P_B] = seed_gene(au[4], c);
+        genes[(c.pop - 3) * M + P_GAMMA] = seed_gene(au[5], c);
+        genes[(c.pop - 3) * M + P_CHI] = seed_gene(au[6], c);
     }
     for (int i = 0; i < c.pop; ++i) f[i] = fitness(&genes[i * M], obs, mu, lambda, L, ln, c, model);
     if (trace) trace[0] = f[argmin(f.data(), c.pop)];

@@ -108,6 +108,10 @@ void pixel_prologue(const double* obs, int L, const GaCfg& c, double out[6]);
 // Semel 1979) of the most Zeeman-sensitive line, in Gauss (signed), and the box coordinates (u_B, u_gamma) of the seeded
 // member, quantised to 10 bits: out[3] = B_los, q_B, q_gamma (q in 0..1023).
 void pixel_seeds(const double* obs, const double* lambda, int L, const Lines& ln, const GaCfg& c, double out[3]);
+// Reading S2: the weak-field member "as in Auer et al. (1977)"; [glo, ghi] = the pixel's inclination box.
+// out: B_los, gamma, chi, B, then the 10-bit box coordinates of (B, gamma, chi).  prologue bit 8, slot P-3 of P0 (pop >= 4).
+void pixel_seed_auer(const double* obs, const double* lambda, int L, const Lines& ln, const GaCfg& c, double glo, double ghi,
+                     double out[7]);
 double decode_gene(float g, double lo, double hi, int log_scale);
 float gene_value(float stored, const GaCfg& c);   // variant 1: 16-bit code -> g = k / 65535 (eq. 5), rounded to binary32
 // Next generation from (genes[pop][NPAR], chi2[pop]) at generation t >= 1 for global pixel id `pixel`.

@@ -29,12 +29,19 @@ FLOP = {"FFMA2": 4, "FMUL2": 2, "FADD2": 2, "FFMA": 2, "FMUL": 1, "FADD": 1}
 SLOTS = {"FFMA2": 2, "FMUL2": 2, "FADD2": 2, "FFMA": 1, "FMUL": 1, "FADD": 1}
 
 
+# The files the counted kernels (ga_invert_kernel, me_synth_kernel) are compiled from.  Host-side code (me_api.cu: validation and
+# descriptors; me_kernels.cu: launch glue and the small hook kernels; me_probe.cu) is deliberately NOT in the hash: an edit
+# there cannot change the instruction mix of the counted kernels, and hashing it would mark good counts stale.
+KERNEL_SOURCES = ["me_device.cuh", "me_inst.cuh", "faddeeva_table.h", "me_launch.h"]
+
+
 def csrc_sha():
-    """sha256 over the sources libme_b200.so is built from (csrc/*.cu, *.cuh, *.h and include/me.h), in name order."""
+    """sha256 over KERNEL_SOURCES, the csrc/me_inst_*.cu instantiation units and include/me.h (ME_MAX_* fix the descriptor
+    layout), in that order."""
     h = hashlib.sha256()
     d = os.path.join(HERE, "csrc")
-    files = sorted(f for f in os.listdir(d) if f.endswith((".cu", ".cuh", ".h")))
-    for f in [os.path.join(d, f) for f in files] + [os.path.join(ROOT, "include", "me.h")]:
+    inst = sorted(f for f in os.listdir(d) if f.startswith("me_inst_") and f.endswith(".cu"))
+    for f in [os.path.join(d, f) for f in KERNEL_SOURCES + inst] + [os.path.join(ROOT, "include", "me.h")]:
         h.update(os.path.basename(f).encode())
         h.update(open(f, "rb").read())
     return h.hexdigest()[:16]
