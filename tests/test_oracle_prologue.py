@@ -144,3 +144,128 @@ def test_seeded_members_enter_the_initial_population():
         cfg["lo"][j] = cfg["hi"][j] = q0[0, j]
     r0 = orc.ga_invert(o0, lam, ln, cfg, seed=5)
     assert r0["genes"][0, 0] == 0.0 and abs(r0["params"][0, 0] - cfg["lo"][0]) < 1e-9
+
+
+# ---- reading S2: the weak-field member "as in Auer et al. (1977)" --------------------------------
+C_ZEEMAN, LAM0, G_EFF = 4.66857e-13, 6302.5017, 2.5
+
+
+def _weak_field_construction(B, gam, chi, step=0.0005, n=801, w=0.030, depth=0.6):
+    """Profiles that obey the weak-field relations EXACTLY by construction, from the analytic derivatives of a Gaussian line:
+    V = -dl_B cos(gamma) I',  (Q, U) = -(1/4) dl_B^2 sin^2(gamma) I'' (cos 2chi, sin 2chi),  dl_B = C g lambda0^2 B."""
+    lam = W.grid(LAM0, n, step)
+    x = lam - LAM0
+    e = depth * np.exp(-x ** 2 / w ** 2)
+    I, I1, I2 = 1.0 - e, e * 2 * x / w ** 2, e * (2 / w ** 2) * (1 - 2 * x ** 2 / w ** 2)
+    dl = C_ZEEMAN * G_EFF * LAM0 ** 2 * B
+    k1, k2 = dl * np.cos(np.radians(gam)), 0.25 * dl ** 2 * np.sin(np.radians(gam)) ** 2
+    obs = np.stack([I, -k2 * np.cos(2 * np.radians(chi)) * I2, -k2 * np.sin(2 * np.radians(chi)) * I2, -k1 * I1])
+    return lam, obs, dl / w
+
+
+def test_auer_seed_inverts_the_weak_field_relations_exactly():
+    # The sharp pin of reading S2: on profiles built from the weak-field relations the seed must return the field they were
+    # built with.  Fixes the assembly: core separation = 2 dl_B cos(gamma) (I + V sees sigma_red: pin P2), the factor 2 and
+    # the square roots of tan(gamma) = 2 sqrt(Lm) D1 / (Vm sqrt(D2)), the sign rule of the azimuth, the atan2 order.
+    # B_los: the core of I - k1 I' sits at k1 (1 - 2 (k1/w)^2 + ...), so the relative error is bounded by 2 (dl_B / w)^2.
+    ln, cfg = single_line(G_EFF, LAM0), W.ga_config(8, 2)
+    for B, gam, chi in [(20, 30, 10), (20, 60, 100), (20, 120, 45), (20, 150, 170), (5, 75, 60), (50, 45, 135), (30, 89, 0), (30, 91, 90)]:
+        lam, obs, ratio = _weak_field_construction(B, gam, chi)
+        o = orc.seed_auer(obs[None], lam, ln, cfg)[0]
+        blos = B * np.cos(np.radians(gam))
+        assert abs(o[0] - blos) <= (2.0 * ratio ** 2 + 1e-3) * abs(blos) + 1e-3, (B, gam, o[0], blos)
+        assert abs(o[1] - gam) < 0.02, (B, gam, o[1])                                    # inclination, degrees
+        d = abs(o[2] - chi) % 180.0
+        assert min(d, 180.0 - d) < 1e-6, (chi, o[2])                                     # azimuth, exact
+        assert abs(o[3] - max(abs(o[0]) / max(abs(np.cos(np.radians(o[1]))), 0.125), cfg["lo"][0])) < 1e-9
+        # the 10-bit box coordinates are the quantised decode of (B, gamma, chi)
+        lo, hi = cfg["lo"], cfg["hi"]
+        assert o[4] == np.rint(1023 * np.log(o[3] / lo[0]) / np.log(hi[0] / lo[0]))
+        assert o[5] == np.rint(1023 * (o[1] - lo[1]) / (hi[1] - lo[1])) and o[6] == np.rint(1023 * (o[2] - lo[2]) / (hi[2] - lo[2]))
+
+
+def test_auer_seed_symmetries_and_polarity_check():
+    ln, cfg = single_line(G_EFF, LAM0), W.ga_config(8, 2)
+    lam, obs, _ = _weak_field_construction(40, 35, 25)
+    a = orc.seed_auer(obs[None], lam, ln, cfg)[0]
+    flip = obs.copy(); flip[3] *= -1                                  # V -> -V: the other polarity
+    b = orc.seed_auer(flip[None], lam, ln, cfg)[0]
+    assert abs(b[0] + a[0]) < 1e-9 and abs(b[1] - (180.0 - a[1])) < 1e-9 and abs(b[2] - a[2]) < 1e-9
+    rot = obs.copy(); rot[1], rot[2] = -obs[2], obs[1]                # (Q, U) rotated by 90 deg = azimuth + 45 deg
+    c = orc.seed_auer(rot[None], lam, ln, cfg)[0]
+    assert abs(((c[2] - a[2]) % 180.0) - 45.0) < 1e-6 and abs(c[1] - a[1]) < 1e-9
+    neg = obs.copy(); neg[1:3] *= -1                                  # (Q, U) -> -(Q, U) = azimuth + 90 deg
+    assert abs(((orc.seed_auer(neg[None], lam, ln, cfg)[0][2] - a[2]) % 180.0) - 90.0) < 1e-6
+    # PAPER.md:278 "the seed fields are checked to ensure that they are consistent with this polarity": with the pixel's
+    # inclination box cut to one polarity the member lies inside it, whatever sign its own B_los estimate has
+    for glo, ghi in ((0.0, 90.0), (90.0, 180.0)):
+        for o in (obs, flip):
+            s = orc.seed_auer(o[None], lam, ln, cfg, glo=[glo], ghi=[ghi])[0]
+            assert glo <= s[1] <= ghi and 0 <= s[5] <= 1023
+    inside = orc.seed_auer(obs[None], lam, ln, cfg, glo=[0.0], ghi=[90.0])[0]
+    assert abs(inside[1] - a[1]) < 1e-9                               # already consistent: untouched
+    outside = orc.seed_auer(flip[None], lam, ln, cfg, glo=[0.0], ghi=[90.0])[0]
+    assert abs(outside[1] - a[1]) < 1e-9                              # reflected back: 180 - (180 - gamma)
+    # unpolarised input: B_los = 0, the member degenerates to the smallest field of the box, no NaN
+    quiet = obs.copy(); quiet[1:] = 0.0
+    z = orc.seed_auer(quiet[None], lam, ln, cfg)[0]
+    assert z[0] == 0.0 and np.all(np.isfinite(z)) and z[4] == 0.0
+
+
+def test_auer_seed_on_synthesised_weak_field_profiles():
+    # What the approximation is worth on real Milne-Eddington profiles (oracle synthesis, 2 mA sampling, no noise).
+    # B_los is THEORY: the core separation equals 2 dl_B cos(gamma) up to O((dl_B / dlambdaD)^2), hence the tight band for
+    # B <= 100 G.  The angle bands are NOT derived: they record the measured quality of Q, U ~ I'' on saturated lines
+    # (eta0 up to 50), where the inclination comes out biased towards 90 deg by up to 11 deg even at 20 G (measured when this
+    # reading was written: |dgamma| <= 11.0 deg, |dchi| <= 3.5 deg for 40 <= gamma <= 140 at B <= 100 G), plus a margin.
+    # A seed needs no more ("at least a few high-quality solutions", PAPER.md:274); it is no substitute for the inversion.
+    ln, cfg = single_line(G_EFF, LAM0), W.ga_config(8, 2)
+    lam = W.grid(LAM0, 401, 0.002)
+    for B in (20.0, 50.0, 100.0):
+        p = W.draw_truth(6, seed=50 + int(B)); p[:, 0] = B; p[:, 6] = 0.3; p[:, 1] = [20, 50, 80, 100, 130, 160]
+        o = orc.seed_auer(orc.synth(p, lam, ln), lam, ln, cfg)
+        blos = B * np.cos(np.radians(p[:, 1]))
+        assert np.all(np.abs(o[:, 0] - blos) <= 0.02 * np.abs(blos)), (B, o[:, 0] / blos)
+        assert np.all(np.sign(o[:, 0]) == np.sign(blos))
+        assert np.all((o[:, 1] < 90.0) == (p[:, 1] < 90.0))                       # the right polarity
+        assert np.max(np.abs(o[:, 1] - p[:, 1])) <= 15.0, o[:, 1] - p[:, 1]
+        mid = (p[:, 1] >= 40) & (p[:, 1] <= 140)
+        d = np.abs(o[mid, 2] - p[mid, 2]) % 180.0
+        assert np.max(np.minimum(d, 180.0 - d)) <= 5.0
+    # at BASELINE config 1's sampling and noise (24 mA, two lines, sigma = 1e-3) it is still a useful start
+    c1 = W.config1()
+    ln2 = oracle_lines(c1["lines"], True)
+    p = W.draw_truth(200, seed=77); p[:, 0] = np.linspace(50, 400, 200)
+    clean = orc.synth(p, c1["lam"], ln2)
+    o = orc.seed_auer(clean + W.draw_noise(clean.shape, 1e-3), c1["lam"], ln2, cfg)
+    blos = p[:, 0] * np.cos(np.radians(p[:, 1]))
+    assert np.median(np.abs(o[:, 0] - blos)) < 0.15 * np.median(np.abs(blos))   # measured 8.3 G on a median |B_los| of 122 G
+    assert np.mean(np.sign(o[:, 0]) == np.sign(blos)) > 0.9                    # measured 0.98
+    assert np.median(np.abs(o[:, 1] - p[:, 1])) < 15.0                         # measured 7.7 deg
+
+
+def test_auer_member_enters_the_initial_population():
+    # prologue bit 8: slot P-3 of P0 holds the quantised (B, gamma, chi) of reading S2.  With the thermodynamic genes fixed
+    # at the truth that member beats 29 random (B, gamma, chi) draws: after ZERO generations the answer is that member.
+    ln = oracle_lines([W.FE_6302])
+    lam = W.grid(W.FE_6302["lambda0"], 50, 0.024)
+    truth = W.draw_truth(8, seed=43)
+    truth[:, 0] = 250.0; truth[:, 1] = np.where(np.arange(8) % 2 == 0, 35.0, 145.0); truth[:, 2] = np.linspace(10, 170, 8)
+    obs = orc.synth(truth, lam, ln) + W.draw_noise((8, 4, 50), 1e-3, stream=3)
+    for variant in (0, 1):
+        won = []
+        for n in range(8):
+            cfg = W.ga_config(32, 0, variant=variant, prologue=8)
+            for j in range(3, 9):
+                cfg["lo"][j] = cfg["hi"][j] = truth[n, j]
+            res = orc.ga_invert(obs[n:n + 1], lam, ln, cfg, seed=2, pixel_base=n)
+            q = orc.seed_auer(obs[n:n + 1], lam, ln, cfg)[0][4:]
+            want = [np.float32(64.0 * x) if variant else np.float32(x) / np.float32(1023.0) for x in q]
+            won.append(all(res["genes"][0, j] == want[j] for j in range(3)))
+            plain = orc.ga_invert(obs[n:n + 1], lam, ln, dict(cfg, prologue=0), seed=2, pixel_base=n)
+            assert plain["chi2"][0] >= res["chi2"][0] or not won[-1]       # without the flag that member cannot be there
+        assert np.mean(won) >= 0.75, (variant, won)
+    # all three seed bits together: slots P-1 (non-magnetic), P-2 (centre of gravity), P-3 (Auer) do not collide
+    cfg = W.ga_config(4, 0, prologue=4 | 8)
+    r = orc.ga_invert(obs[:1], lam, ln, cfg, seed=2)
+    assert np.isfinite(r["chi2"][0])
