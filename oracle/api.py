@@ -105,8 +105,16 @@ def prologue(obs, cfg):
     return out
 
 
-def uncertainty(obs, params, lam, lines, cfg, mu=None, nm_profile=None, threads=1):
-    """eq. 26 / reading U1: obs[N,4,L], params[N,M] (the optimum) -> (sigma[N,M], chi2[N])."""
+def uncertainty_step():
+    """The finite-difference step h of reading U1, in box coordinates."""
+    f = lib().orc_uncertainty_step
+    f.restype = C.c_double
+    return float(f())
+
+
+def uncertainty(obs, params, lam, lines, cfg, mu=None, nm_profile=None, threads=1, want_hessian=False):
+    """eq. 26 / reading U1: obs[N,4,L], params[N,M] (the optimum) -> (sigma[N,M], chi2[N]) and, if asked, the Hessians
+    [N,M,M] in box coordinates."""
     obs, lam, params = _f64(obs), _f64(lam), _f64(params)
     N, L, npar = obs.shape[0], lam.size, _npar(cfg)
     assert params.shape == (N, npar)
@@ -115,11 +123,13 @@ def uncertainty(obs, params, lam, lines, cfg, mu=None, nm_profile=None, threads=
     lo, hi, lg = _f64(cfg["lo"]), _f64(cfg["hi"]), _i32(cfg["log_scale"])
     w, sg = _f64(cfg["stokes_weight"]), _f64(cfg["sigma"])
     sig, chi = np.empty((N, npar)), np.empty(N)
+    hess = np.empty((N, npar, npar)) if want_hessian else None
     lib().orc_uncertainty(_p(obs, C.c_double), _p(mu_a, C.c_double), C.c_int64(N), _p(lam, C.c_double), C.c_int(L),
                           *lines.args(), _p(lo, C.c_double), _p(hi, C.c_double), _p(lg, C.c_int), _p(w, C.c_double),
                           _p(sg, C.c_double), C.c_int(npar), C.c_int(int(cfg.get("prologue", 0))), _p(nm, C.c_double),
-                          _p(params, C.c_double), C.c_int(threads), _p(sig, C.c_double), _p(chi, C.c_double))
-    return sig, chi
+                          _p(params, C.c_double), C.c_int(threads), _p(sig, C.c_double), _p(chi, C.c_double),
+                          _p(hess, C.c_double))
+    return (sig, chi, hess) if want_hessian else (sig, chi)
 
 
 def uncertainty_n_eval(M):

@@ -103,20 +103,21 @@ void orc_prologue(const double* obs, int64_t N, int L, const double* w, const do
     for (int64_t n = 0; n < N; ++n) pixel_prologue(obs + n * 4 * L, L, c, out + n * 6);
 }
 
-// Uncertainties (reading U1). params[N][npar] -> sigma_out[N][npar], chi2_out[N] (may be null).
+// Uncertainties (reading U1). params[N][npar] -> sigma_out[N][npar], chi2_out[N], hess_out[N][npar][npar] (each may be null).
+double orc_uncertainty_step() { return UNC_H; }
 void orc_uncertainty(const double* obs, const double* mu, int64_t N, const double* lambda, int L,
                      int n_lines, const double* lambda0, const double* strength, const int* n_comp,
                      const double* shift, const double* weight, const int* kind, double lambda_ref,
                      const double* lo, const double* hi, const int* log_scale, const double* w, const double* sigma,
                      int npar, int prologue, const double* nm_profile, const double* params, int threads,
-                     double* sigma_out, double* chi2_out) {
+                     double* sigma_out, double* chi2_out, double* hess_out /* [N][npar][npar] or null */) {
     Lines ln = make_lines(n_lines, lambda0, strength, n_comp, shift, weight, kind, lambda_ref);
     GaCfg c; c.npar = npar; c.nm_profile = nm_profile; c.prologue = prologue;
     for (int j = 0; j < npar; ++j) { c.lo[j] = lo[j]; c.hi[j] = hi[j]; c.log_scale[j] = log_scale[j]; c.periodic[j] = 0; }
     for (int s = 0; s < 4; ++s) { c.w[s] = w[s]; c.sigma[s] = sigma[s]; }
     parallel_for(N, threads, [&](int64_t n) {
         uncertainty_pixel(obs + n * 4 * L, mu ? mu[n] : 1.0, lambda, L, ln, c, params + n * npar, sigma_out + n * npar,
-                          chi2_out ? chi2_out + n : nullptr);
+                          chi2_out ? chi2_out + n : nullptr, hess_out ? hess_out + n * npar * npar : nullptr);
     });
 }
 

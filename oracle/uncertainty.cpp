@@ -6,7 +6,7 @@
 // "bootstrap[ped] to higher accuracy by Richardson extrapolation to zero stepsize within Neville's algorithm".
 // The paper starts from a population-based gradient (eq. 25) whose choice of members it does not specify; reading U1
 // of DESIGN.md takes the deterministic equivalent: central second differences of chi2 on the box coordinates
-// u in [0,1]^M (p = decode(u), reading G1) at steps h = 2^-7 and h/2, one Neville/Richardson level
+// u in [0,1]^M (p = decode(u), reading G1) at steps h = UNC_H = 2^-6 and h/2, one Neville/Richardson level
 //     D = (4 D(h/2) - D(h)) / 3,
 //     D_jj(h) = [chi2(u + h e_j) - 2 chi2(u) + chi2(u - h e_j)] / h^2,
 //     D_jk(h) = [chi2(++) - chi2(+-) - chi2(-+) + chi2(--)] / (4 h^2),
@@ -63,7 +63,9 @@ static bool invert(std::vector<double>& a, int n) {
 }
 
 // chi2v[n_eval] in the order of uncertainty_offsets -> sigma_u[M] (NaN on failure); active[j] = 0 leaves gene j out.
-void uncertainty_from_chi2(const double* chi2v, int M, double h, const int* active, double* sigma_u) {
+// hess_out (optional): the M x M Richardson-extrapolated Hessian in box coordinates, all genes (tests use its eigenvalues
+// to say how well-posed eq. 26 is for a pixel).
+void uncertainty_from_chi2(const double* chi2v, int M, double h, const int* active, double* sigma_u, double* hess_out) {
     const int per_level = 2 * M + 2 * M * (M - 1);
     std::vector<double> H(M * M, 0.0);
     for (int j = 0; j < M; ++j)
@@ -83,6 +85,7 @@ void uncertainty_from_chi2(const double* chi2v, int M, double h, const int* acti
             }
             H[j * M + k] = H[k * M + j] = (4.0 * D[1] - D[0]) / 3.0;          // Richardson / Neville, one level
         }
+    if (hess_out) for (int q = 0; q < M * M; ++q) hess_out[q] = H[q];
     std::vector<int> idx;
     for (int j = 0; j < M; ++j) if (active[j]) idx.push_back(j);
     const int n = (int)idx.size();
@@ -98,7 +101,7 @@ void uncertainty_from_chi2(const double* chi2v, int M, double h, const int* acti
 }
 
 void uncertainty_pixel(const double* obs, double mu, const double* lambda, int L, const Lines& ln, const GaCfg& c0,
-                       const double* params, double* sigma_p, double* chi2_opt) {
+                       const double* params, double* sigma_p, double* chi2_opt, double* hess_out) {
     GaCfg c = c0;
     if (c0.prologue) {
         double pr[6];
@@ -107,7 +110,7 @@ void uncertainty_pixel(const double* obs, double mu, const double* lambda, int L
         c.lo[P_GAMMA] = pr[4]; c.hi[P_GAMMA] = pr[5];
     }
     const int M = c.npar;
-    const double h = 1.0 / 128.0;
+    const double h = UNC_H;
     std::vector<double> u0(M), p(M), du, model(4 * L);
     std::vector<int> active(M);
     for (int j = 0; j < M; ++j) {
@@ -128,7 +131,7 @@ void uncertainty_pixel(const double* obs, double mu, const double* lambda, int L
         chi2v[e] = chi2(obs, model.data(), L, c.w, c.sigma, M);
     }
     std::vector<double> su(M);
-    uncertainty_from_chi2(chi2v.data(), M, h, active.data(), su.data());
+    uncertainty_from_chi2(chi2v.data(), M, h, active.data(), su.data(), hess_out);
     for (int j = 0; j < M; ++j) {
         const double dpdu = c.log_scale[j] ? params[j] * std::log(c.hi[j] / c.lo[j]) : (c.hi[j] - c.lo[j]);
         sigma_p[j] = su[j] * std::fabs(dpdu);

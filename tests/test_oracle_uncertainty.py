@@ -7,7 +7,7 @@ from helpers import oracle_lines
 from oracle import api as orc
 from paper_1208_0302_b200 import workloads as W
 
-H_STEP = 1.0 / 128.0
+H_STEP = orc.uncertainty_step()          # reading U1: 2^-6
 
 
 def _table(f, M, u0):
@@ -91,3 +91,29 @@ def test_noiseless_profile_gives_the_gauss_newton_hessian():
     # sigma scales with the noise level (H is noise-independent to first order, chi2 is quadratic in it)
     sig2, _ = orc.uncertainty(obs + 2.0 * (noisy - obs), truth, lam, ln, cfg)
     assert np.allclose(sig2 / sig, 2.0, rtol=0.1)
+
+
+def test_returned_hessian_is_the_one_eq_26_inverts():
+    # uncertainty(..., want_hessian=True) hands out the Richardson-extrapolated Hessian in box coordinates: eq. 26 applied to
+    # it with numpy's inverse reproduces the returned sigmas, it is symmetric, and asking for it changes nothing else
+    c0 = W.config0()
+    ln = oracle_lines(c0["lines"], True)
+    truth = W.draw_truth(6, seed=31)
+    truth[:, 0] = np.maximum(truth[:, 0], 900.0)
+    obs = orc.synth(truth, c0["lam"], ln) + W.draw_noise((6, 4, c0["lam"].size), 1e-3, stream=9)
+    cfg = c0["ga"]
+    sig, chi, H = orc.uncertainty(obs, truth, c0["lam"], ln, cfg, threads=6, want_hessian=True)
+    sig2, chi2 = orc.uncertainty(obs, truth, c0["lam"], ln, cfg, threads=6)
+    assert np.array_equal(np.nan_to_num(sig), np.nan_to_num(sig2)) and np.array_equal(chi, chi2)
+    assert H.shape == (6, 9, 9) and np.allclose(H, np.transpose(H, (0, 2, 1)), rtol=0, atol=0)
+    lo, hi = np.asarray(cfg["lo"]), np.asarray(cfg["hi"])
+    with np.errstate(all="ignore"):                                            # the log is only taken where the gene is log-scaled
+        dpdu = np.where(cfg["log_scale"], truth * np.log(hi / lo), hi - lo)
+    seen = 0
+    for n in range(6):
+        if not np.all(np.isfinite(sig[n])):
+            continue
+        su = np.sqrt(np.diag(np.linalg.inv(H[n])) * chi[n] / 9.0)              # eq. 26
+        assert np.allclose(su * np.abs(dpdu[n]), sig[n], rtol=1e-9)
+        seen += 1
+    assert seen >= 3
