@@ -132,6 +132,10 @@ typedef struct {
                                     (reading S1): B = |B_los| from the centre of gravity of I +- V
                                     (Rees & Semel 1979) with gamma at the matching end of its box, and the non-magnetic
                                     solution B = lo[0]; other genes as drawn. Needs pop >= 3.
+                                 8: the weak-field member "as in Auer et al. (1977)" (reading S2)
+                                    takes slot pop-3: B_los from the separation of the I+V and I-V line cores, azimuth
+                                    and inclination from the maxima of Q^2+U^2, |V| and the derivatives of I, reflected
+                                    into the (polarity-cut) inclination box, B = |B_los| / |cos gamma|. Needs pop >= 4.
                                  ga_fitness ignores these flags (fixed weights, configured box). */
 } ga_cfg;
 
@@ -146,7 +150,7 @@ int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sig
               float* out_params, float* out_chi2, void* stream);
 
 /* Parameter uncertainties at the optimum (eq. 26; reading U1): the Hessian H of chi2 on the
- * box coordinates (central second differences at h = 2^-7 and h/2, one Richardson/Neville level; 1 + 2(2M + 2M(M-1))
+ * box coordinates (central second differences at h = 2^-6 and h/2, one Richardson/Neville level; 1 + 2(2M + 2M(M-1))
  * syntheses per pixel through the same fused fitness as ga_invert), sigma_i^2 = [H^-1]_ii chi2(p_opt)/M, scaled to
  * parameter units. Genes with lo == hi are left out (sigma = 0). A singular or indefinite Hessian gives NaN.
  *   params     device [N, n_params] f32: the optimum (ga_invert's out_params)
@@ -164,8 +168,9 @@ int ga_step(const float* genes_in /*[N,pop,n_params]*/, const float* chi2_in /*[
 int ga_fitness(const float* genes /*[N,pop,n_params]*/, const float* obs /*[N,4,L]*/, int64_t N, const float* sigma /*host[4]*/,
                const double* lambda_grid_A, int L, const me_line_data* line_data, const ga_cfg* cfg,
                float* chi2_out /*[N,pop]*/, void* stream);
-/* The per-pixel prologue alone: out device [N,9] f32 = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them,
- * then B_los [G] and the stored genes (B, gamma) of the centre-of-gravity member (0 unless prologue bit 4). */
+/* The per-pixel prologue alone: out device [N,12] f32 = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them,
+ * then B_los [G] and the stored genes (B, gamma) of the centre-of-gravity member (0 unless prologue bit 4), then the stored
+ * genes (B, gamma, chi) of the Auer weak-field member (0 unless prologue bit 8).  Allocates nothing, does not synchronise. */
 int ga_prologue(const float* obs /*[N,4,L]*/, int64_t N, const float* sigma /*host[4]*/, const double* lambda_grid_A, int L,
                 const me_line_data* line_data, const ga_cfg* cfg, float* out, void* stream);
 /* Generation-0 population (reading G2): genes_out device [N,pop,n_params]. */
@@ -180,8 +185,8 @@ int me_faddeeva(const float* v, const float* a, int64_t n, float* H, float* F, v
 
 /* Instruction-throughput probe for the roofline denominators (SURVEY.md par. 8(d)): launches `blocks` CTAs of 256
  * threads, each thread running `iters` x 32 slots of one instruction class in 8 independent register chains.
- * kind: 0 FFMA, 1 FFMA2 (packed fp32x2), 2 FFMA2+FFMA 1:1, 3 MUFU.RCP, 4 FMUL2, 5 FFMA2+FFMA 2:1, 6 FFMA2+MUFU 8:1,
- *       7-9 FFMA2 operand forms (pair*scalar+scalar, pair*pair+imm, pair*scalar+pair), 10 FADD2.
+ * kind: 0 FFMA (scalar), 1 FFMA2 (packed fp32x2, the form the fitness loop is written in), 3 MUFU.RCP/EX2; any other
+ *       value is ME_ERR_CUDA (invalid value).
  * out: device [blocks*256] f32 scratch (never written in practice). The caller times the call with CUDA events. */
 int me_peak_probe(int kind, int iters, int blocks, float* out, void* stream);
 

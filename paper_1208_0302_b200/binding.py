@@ -284,14 +284,15 @@ def me_peak_probe(kind, iters, blocks, scratch):
 
 
 def ga_prologue(obs, lam, line_data, cfg):
-    """obs: CUDA f32 [N,4,L]. Returns [N,9]: w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them, then B_los [G] and
-    the stored genes (B, gamma) of the centre-of-gravity member (cfg["prologue"] bit flags)."""
+    """obs: CUDA f32 [N,4,L]. Returns [N,12]: w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi as ga_invert uses them, then B_los [G] and
+    the stored genes (B, gamma) of the centre-of-gravity member, then the stored genes (B, gamma, chi) of the Auer weak-field
+    member (cfg["prologue"] bit flags 4 and 8)."""
     import torch
     N = obs.shape[0]
     lam, lam_p, L = _grid(lam)
     c, keep = make_ga_cfg(cfg)
     sig = np.ascontiguousarray(cfg["sigma"], dtype=np.float32)
-    out = torch.empty((N, 9), dtype=torch.float32, device=obs.device)
+    out = torch.empty((N, 12), dtype=torch.float32, device=obs.device)
     _check(lib().ga_prologue(_dev(obs, torch.float32, "obs"), C.c_int64(N), sig.ctypes.data_as(C.POINTER(C.c_float)), lam_p, L,
                              C.byref(line_data.c), C.byref(c), _dev(out, torch.float32, "out"), _stream()), "ga_prologue")
     return out

@@ -106,9 +106,10 @@ int build_ga_desc(const ga_cfg* c, int npar, const float* sigma, int L, uint64_t
         if (c->elite != 1) return ME_ERR_UNSUPPORTED;
         if (!(c->p_cross >= 0.f && c->p_cross <= 1.f) || !(c->p_mut >= 0.f && c->p_mut <= 1.f)) return ME_ERR_RANGE;
         if ((c->prologue & 4) && c->pop < 3) return ME_ERR_SHAPE;             // reading S1: the seeds take the last two slots of P0
+        if ((c->prologue & 8) && c->pop < 4) return ME_ERR_SHAPE;             // reading S2: the Auer member takes slot P-3
     }
     if (c->variant != 0 && c->variant != 1) return ME_ERR_RANGE;
-    if (c->prologue < 0 || c->prologue > 7) return ME_ERR_RANGE;
+    if (c->prologue < 0 || c->prologue > 15) return ME_ERR_RANGE;
     if ((c->prologue & 2) && c->log_scale[1]) return ME_ERR_UNSUPPORTED;      // the polarity box is linear in gamma
     if (c->pixel_id_base < 0 || N < 0 || (uint64_t)c->pixel_id_base + (uint64_t)N > 0x100000000ULL) return ME_ERR_RANGE;
     std::memset(&g, 0, sizeof(g));
@@ -288,7 +289,7 @@ int ga_prologue(const float* obs, int64_t N, const float* sigma, const double* l
     fill_seed_desc(line_data, gd);
     if (N == 0) return ME_OK;
     if (obs == nullptr || out == nullptr) return ME_ERR_NULL;
-    cudaError_t e = me::launch_ga_prologue(&sd, gd, obs, N, L, out, (cudaStream_t)stream);
+    cudaError_t e = me::launch_ga_prologue(sd, gd, obs, N, out, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
 }
 

@@ -67,7 +67,7 @@ struct GaDesc {
 // ------------------------------------------------------------------------------------------------------------
 // Packed FP32 helpers.  Blackwell (sm_100) issues two FP32 FMAs per instruction (FFMA2 / FMUL2 / FADD2); the FMA
 // pipe is as wide as before, so packing halves the ISSUE slots of the arithmetic.  The fitness loop is issue-bound
-// (profiles/r1a), so everything per wavelength is written on pairs of adjacent wavelengths (j, j+1) held in float2.
+// (profiles/r1_history.md, step r1a), so everything per wavelength is written on pairs of adjacent wavelengths (j, j+1) held in float2.
 // Scalars broadcast for free (SASS operand form R.F32), negation is an operand modifier.
 // ------------------------------------------------------------------------------------------------------------
 typedef float2 f2;
@@ -116,7 +116,7 @@ MEDEV FadConst fad_const(float a) {
 // and |s|^2 = r = 1/|z|^2:   w = i s R = r [ a (b0 + r b1) + i v (b0 - r b1) ]   (no cancellation in H).
 // K = number of series terms beyond the leading one: 5 for |z| >= FAD_CUT, 2 for >= FAD_FAR (used as written only when
 // a > FAD_FAR_AMAX; otherwise the far tier below).  An intermediate K = 3 tier (|z| >= 7.5) was measured and dropped: it
-// saved 0.7 % of the arithmetic and cost more than that in code size (profiles/r1e).
+// saved 0.7 % of the arithmetic and cost more than that in code size (profiles/r1_history.md, step r1e).
 template <int K>
 MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
     const f2 r = rcp2(r2);                                    // 1/|z|^2
@@ -147,7 +147,7 @@ MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
 //   F = v r Y(r),  Y = C0 +   C1 r + (  C2 - 4 a^2 C1) r^2 - 12 a^2 C2 r^3 + 16 a^4 C2 r^4
 // (the r^4 terms are < 1e-8 relative for a <= FAD_FAR_AMAX; the r^3 terms are < 3e-6 relative = 1e-8 absolute in H and
 // 5e-8 in F, below the FP32 rounding of the evaluation itself: both are dropped, X and Y are evaluated as quadratics).  The coefficients depend on the individual
-// only, so each Horner step is FFMA2 (pair x pair + scalar) -- the full-rate operand form (profiles/r1c peaks: an
+// only, so each Horner step is FFMA2 (pair x pair + scalar) -- the full-rate operand form (profiles/r1_history.md, step r1c: an
 // FFMA2 whose ADDEND is a register pair runs at 0.77 of that rate) -- and the line strength r_l and the factor a are
 // folded into them:  fx = a r_l (x2, x1, C0),  fy = r_l (y2, y1, C0).
 struct FarCoef { float x2, x1, x0, y2, y1, y0; };
@@ -172,17 +172,22 @@ MEDEV void faddeeva_far_acc(f2 v, f2 r2, const FarCoef& c, f2& sr, f2& si) {
 
 // The same coefficients parked in shared memory (one float4 pair per thread and line) and re-loaded inside the far branch:
 // in registers they do not fit next to the fitness loop's working set and the compiler rematerialises them with ~13
-// scalar FMULs per line and pair on the FMA pipe (profiles/r1e); an LDS.128 pair costs no FMA-pipe slot.
-MEDEV FarCoef far_load(const float4* p, int stride) {
+// scalar FMULs per line and pair on the FMA pipe (profiles/r1_history.md, step r1e); an LDS.128 pair costs no FMA-pipe slot.
+MEDEV FarCoef far_load(unsigned addr, int stride_bytes) {
     float4 x, y;
-    const unsigned ax = (unsigned)__cvta_generic_to_shared(p), ay = (unsigned)__cvta_generic_to_shared(p + stride);
-    // "memory": the compiler must not sink or drop far_store's plain stores, which only these loads read
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(ax) : "memory");
-    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(y.x), "=f"(y.y) : "r"(ay) : "memory");
+    // "memory": the compiler must not sink or drop far_store's plain stores, which only these loads read.  addr is this
+    // thread's column as a 32-bit shared address held in a register (keep_in_register below); stride_bytes is a constant.
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(addr) : "memory");
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(y.x), "=f"(y.y) : "r"(addr + stride_bytes) : "memory");
     FarCoef c;
     c.x2 = x.x; c.x1 = x.y; c.x0 = x.z; c.y2 = x.w; c.y1 = y.x; c.y0 = y.y;
     return c;
 }
+// A loop-invariant value the compiler would otherwise RE-COMPUTE inside the wavelength loop to save a register (ncu r2c:
+// S2R + LEA + 3 moves per far-tier branch for the shared address, FSETP + MOV + FSEL per pair for the far threshold =
+// 6.4 of 112 instructions per wavelength point).  An empty asm with the value as in/out operand makes it opaque.
+MEDEV void keep_in_register(unsigned& x) { asm volatile("" : "+r"(x)); }
+MEDEV void keep_in_register(float& x) { asm volatile("" : "+f"(x)); }
 MEDEV void far_store(float4* p, int stride, const FarCoef& c) {
     p[0] = make_float4(c.x2, c.x1, c.x0, c.y2);
     *reinterpret_cast<float2*>(p + stride) = make_float2(c.y1, c.y0);
@@ -222,22 +227,23 @@ template <int NL>
 struct Individual {
     FadConst fad;
     FarCoef far[NL];                  // far-tier polynomial coefficients per line (strength and a folded in)
-    float far2;                       // |z|^2 threshold of the far tier (+Inf when a > FAD_FAR_AMAX)
+    float tfar;                       // far-tier threshold on dv = min|v| - g vB: FAD_FAR, or +Inf when a > FAD_FAR_AMAX
     float invD[NL], v0[NL], vB[NL];   // 1/dlambdaD_l, -doppler_l/dlambdaD_l, Zeeman splitting in Doppler units
     float kA, kB, kC;                 // h sin^2(gamma), h (1 + cos^2 gamma)/2, h cos(gamma);  h = eta0 / (2 sqrt(pi))
     float c2x, s2x;                   // cos 2chi, sin 2chi
     float S0, muS1;                   // 11-parameter model: (1-s) S0 and (1-s) alpha mu S1
     float k0, nmS1, stray;            // 11-parameter model only: eta0/sqrt(pi), (1-s)(1-alpha) mu S1, s
-    float4* far_s;                    // FARS: this thread's far coefficients in shared memory, [2 l + {0,1}] * far_stride
-    int far_stride;
+    unsigned far_addr;                // FARS: 32-bit shared address of this thread's far coefficients, [2 l + {0,1}] * far_stride
+    int far_stride;                   //       stride in BYTES between consecutive float4 rows (16 * threads per block)
 };
 
 // p: decoded parameter vector, M = 9 or 11 entries.  For M = 11 (reading F13)
 //   I = (1-s)[alpha I^M + (1-alpha) I(B=0)] + s I_fixed
 //     = (1-s) S0 + [(1-s) alpha mu S1] (K^-1 e)_I + [(1-s)(1-alpha) mu S1] / (1 + eta0 phi_nm) + s I_fixed,
 // and Q, U, V carry the factor (1-s) alpha: both are obtained by rescaling S0 and mu S1 here.
+// triplet: ind.vB[l] holds g_l vB_l, the sigma shift itself (the only form the triplet path uses; r2d: one FMUL per line and pair)
 template <int NL, int M>
-MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const SynthDesc& d) {
+MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const SynthDesc& d, bool triplet = false) {
     const float B = p[0], eta0 = p[3], dld = p[4], a = p[5], vlos = p[6];
     float sg, cg;
     sincospif(p[1] * (1.0f / 180.0f), &sg, &cg);
@@ -247,7 +253,8 @@ MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const
     ind.kB = h * 0.5f * fmaf(cg, cg, 1.0f);
     ind.kC = h * cg;
     ind.fad = fad_const(a);
-    ind.far2 = a <= FAD_FAR_AMAX ? FAD_FAR2 : __int_as_float(0x7f800000);
+    ind.tfar = a <= FAD_FAR_AMAX ? FAD_FAR : __int_as_float(0x7f800000);
+    keep_in_register(ind.tfar);
     ind.S0 = p[7];
     ind.muS1 = mu * p[8];
     ind.k0 = ind.nmS1 = ind.stray = 0.f;
@@ -267,26 +274,30 @@ MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const
         ind.invD[l] = inv;
         ind.v0[l] = -(d.line[l].lam0_over_c * vlos) * inv;
         ind.vB[l] = d.line[l].zeeman * B * inv;
+        if (triplet) ind.vB[l] *= d.line[l].g;
     }
 }
 
 // Profile sums of one line at a pair of reduced wavelengths v:
 //   S_kind += r_l * sum_c weight_c * w(v - shift_c vB + i a)
 template <bool TRIPLET, bool FARS>
-MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far_r, const float4* far_s, int far_stride,
-                         float far2, const SynthDesc& d, int l, f2& br, f2& bi, f2& pr, f2& pi, f2& rr, f2& ri) {
+MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far_r, unsigned far_addr, int far_stride,
+                         float tfar, const SynthDesc& d, int l, f2& br, f2& bi, f2& pr, f2& pi, f2& rr, f2& ri) {
     const float r = d.line[l].strength;
     if (TRIPLET) {
-        const float gvB = d.line[l].g * vB;
+        const float gvB = vB;                                      // g vB, formed once per individual (setup_individual)
         f2 w0r, w0i, w1r, w1i, w2r, w2i;
         const f2 vb = add2(v, bc(gvB)), vr = add2(v, bc(-gvB));   // sigma_blue sits at v = -g vB, sigma_red at +g vB
-        const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
-        const float rmin = fminf(fminf(fminf(r2p.x, r2p.y), fminf(r2b.x, r2b.y)), fminf(r2r.x, r2r.y));
+        // Tier of the whole line at this pair: the three components sit at 0, -+g vB, so the one nearest to either
+        // wavelength is at distance >= dv = min(|v.x|, |v.y|) - g vB, and dv >= T guarantees |z| >= T for all six arguments.
+        // (r2c: the minimum over the six |z|^2 cost 3 FMNMX + up to 4 FSETP per line and pair; this is 1 FMNMX + 1 FADD.)
+        const float dv = fminf(fabsf(v.x), fabsf(v.y)) - gvB;
         // When all six arguments lie in one wing tier (the common case) the three evaluations are independent
         // straight-line code that the scheduler interleaves; the series shortens with distance from the line.
-        if (rmin >= far2) {
-            const FarCoef far = FARS ? far_load(far_s + 2 * l * far_stride, far_stride) : far_r;
-            if (rmin >= 400.0f) {
+        if (dv >= tfar) {
+            const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
+            const FarCoef far = FARS ? far_load(far_addr + 2 * l * far_stride, far_stride) : far_r;
+            if (dv >= FAD_FAR_LIN) {
                 faddeeva_far_acc<true>(v, r2p, far, pr, pi);
                 faddeeva_far_acc<true>(vb, r2b, far, br, bi);
                 faddeeva_far_acc<true>(vr, r2r, far, rr, ri);
@@ -297,11 +308,13 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
             }
             return;
         }
-        if (rmin >= FAD_FAR2) {                                   // a > FAD_FAR_AMAX: the series itself
+        if (dv >= FAD_FAR) {                                      // a > FAD_FAR_AMAX: the series itself
+            const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
             faddeeva_wing<2>(v, r2p, fad, w0r, w0i);
             faddeeva_wing<2>(vb, r2b, fad, w1r, w1i);
             faddeeva_wing<2>(vr, r2r, fad, w2r, w2i);
-        } else if (rmin >= FAD_CUT2) {
+        } else if (dv >= FAD_CUT) {
+            const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
             faddeeva_wing<5>(v, r2p, fad, w0r, w0i);
             faddeeva_wing<5>(vb, r2b, fad, w1r, w1i);
             faddeeva_wing<5>(vr, r2r, fad, w2r, w2i);
@@ -318,10 +331,9 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
         // line centre, so the smallest |z|^2 over all of them and both wavelengths is bounded below by
         // (max(0, min|v| - smax |vB|))^2 + a^2: one tier for the whole line, chosen without touching the components.
         const int* kb = d.line[l].kind_begin;
-        const float dmin = fmaxf(fminf(fabsf(v.x), fabsf(v.y)) - d.line[l].smax * fabsf(vB), 0.0f);
-        const float rmin = fmaf(dmin, dmin, fad.a2);
+        const float dv = fminf(fabsf(v.x), fabsf(v.y)) - d.line[l].smax * fabsf(vB);
         const FarCoef far = far_r;
-        const int tier = rmin >= far2 ? 2 : (rmin >= FAD_CUT2 ? 1 : 0);
+        const int tier = dv >= tfar ? 2 : (dv >= FAD_CUT ? 1 : 0);
 #pragma unroll 1
         for (int k = 0; k < 3; ++k) {                              // k = 0 blue, 1 pi, 2 red
             f2 ar = bc(0.f), ai = bc(0.f);
@@ -359,7 +371,9 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
 // The Unno-Rachkovsky solution is evaluated in the frame chi = 0 (eta_U = rho_U = 0) and Q,U are rotated by 2 chi.
 // M = 11: nmF = I_fixed at the two wavelengths; the field-free profile sum phi_nm = sum_l r_l H(a, v_l) is the pi sum of
 // effective triplets (their pi component is unshifted with weight 1), else one extra Voigt per line.
-template <int NL, bool TRIPLET, int M, bool FARS = false>
+// RES: on entry I, Q, U, V hold the OBSERVED values at the pair; on return they hold the residuals observed - model, formed
+// by the last FMA of each Stokes parameter instead of a separate subtraction (the fused fitness needs nothing else).
+template <int NL, bool TRIPLET, int M, bool FARS = false, bool RES = false>
 MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2 nmF, f2& I, f2& Q, f2& U, f2& V,
                        const f2* offp = nullptr) {
     f2 br = bc(0.f), bi = bc(0.f), pr = bc(0.f), pi = bc(0.f), rr = bc(0.f), ri = bc(0.f), nr = bc(0.f);
@@ -368,7 +382,7 @@ MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bo
         if (NL == ME_MAX_LINES && l >= d.n_lines) break;      // NL == ME_MAX_LINES is the run-time-sized fallback
         const f2 off = offp != nullptr ? offp[l] : (tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]));
         const f2 v = fma2(ind.invD[l], off, ind.v0[l]);
-        line_profiles<TRIPLET, FARS>(v, ind.vB[l], ind.fad, ind.far[l], ind.far_s, ind.far_stride, ind.far2, d, l, br, bi,
+        line_profiles<TRIPLET, FARS>(v, ind.vB[l], ind.fad, ind.far[l], ind.far_addr, ind.far_stride, ind.tfar, d, l, br, bi,
                                      pr, pi, rr, ri);
         if (M == ME_MAX_NPAR && !TRIPLET) {
             f2 wr, wi;
@@ -383,21 +397,37 @@ MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bo
     const f2 rL = mul2(ind.kA, fma2(-0.5f, si, pi));              // rho_Q in the chi = 0 frame
     const f2 eV = mul2(ind.kC, sub2(rr, br));
     const f2 rV = mul2(ind.kC, sub2(ri, bi));
-    const f2 eI2 = mul2(eI, eI);
+    // r2d: this tail is the largest consumer of the FMA pipe, which limits the kernel (31 % of its lane-slots, two thirds of
+    // them bare FMUL2 / FADD2).  eI^2 + rho^2 and eI^2 + rho^2 - eta^2 are formed by chained FMAs, -mu S1 eI / Delta is shared
+    // between I and U, and in RES mode the subtraction from the observation is the last FMA of each Stokes parameter.
+    const f2 E2 = mul2(eI, eI);
+    const f2 A = fma2(rL, rL, fma2(rV, rV, E2));                  // eta_I^2 + rho_Q^2 + rho_V^2
+    const f2 Bq = fma2(neg(eL), eL, fma2(neg(eV), eV, A));        // ... - eta_Q^2 - eta_V^2
     const f2 Pi = fma2(eL, rL, mul2(eV, rV));
-    const f2 rho2 = fma2(rL, rL, mul2(rV, rV));
-    const f2 eta2 = fma2(eL, eL, mul2(eV, eV));
-    const f2 Delta = fma2(eI2, add2(eI2, sub2(rho2, eta2)), neg(mul2(Pi, Pi)));
+    const f2 Delta = fma2(E2, Bq, neg(mul2(Pi, Pi)));
     const f2 nt = mul2(-ind.muS1, rcp2(Delta));                   // -mu S1 / Delta
-    I = fma2(mul2(neg(nt), eI), add2(eI2, rho2), ind.S0);
-    const f2 Qp = mul2(nt, fma2(eI2, eL, mul2(rL, Pi)));
-    const f2 Up = mul2(mul2(nt, eI), fma2(eL, rV, neg(mul2(eV, rL))));
-    V = mul2(nt, fma2(eI2, eV, mul2(rV, Pi)));
-    Q = fma2(ind.c2x, Qp, mul2(-ind.s2x, Up));
-    U = fma2(ind.s2x, Qp, mul2(ind.c2x, Up));
-    if (M == ME_MAX_NPAR) {
-        const f2 rn = rcp2(fma2(ind.k0, nr, 1.0f));               // 1 / (1 + eta0 phi_nm): pin P1
-        I = fma2(ind.nmS1, rn, fma2(ind.stray, nmF, I));
+    const f2 nteI = mul2(nt, eI);
+    const f2 Qp = mul2(nt, fma2(E2, eL, mul2(rL, Pi)));
+    const f2 Up = mul2(nteI, fma2(eL, rV, neg(mul2(eV, rL))));
+    const f2 Vn = fma2(E2, eV, mul2(rV, Pi));
+    if (!RES) {
+        I = fma2(neg(nteI), A, ind.S0);
+        V = mul2(nt, Vn);
+        Q = fma2(ind.c2x, Qp, mul2(-ind.s2x, Up));
+        U = fma2(ind.s2x, Qp, mul2(ind.c2x, Up));
+        if (M == ME_MAX_NPAR) {
+            const f2 rn = rcp2(fma2(ind.k0, nr, 1.0f));           // 1 / (1 + eta0 phi_nm): pin P1
+            I = fma2(ind.nmS1, rn, fma2(ind.stray, nmF, I));
+        }
+    } else {
+        I = add2(fma2(nteI, A, I), bc(-ind.S0));                  // obs_I - (S0 - nt eI A)
+        V = fma2(neg(nt), Vn, V);
+        Q = fma2(-ind.c2x, Qp, fma2(ind.s2x, Up, Q));
+        U = fma2(-ind.s2x, Qp, fma2(-ind.c2x, Up, U));
+        if (M == ME_MAX_NPAR) {
+            const f2 rn = rcp2(fma2(ind.k0, nr, 1.0f));
+            I = fma2(-ind.nmS1, rn, fma2(-ind.stray, nmF, I));
+        }
     }
 }
 
@@ -599,7 +629,7 @@ __device__ __forceinline__ void stage_obs(float* obs_s, const float* obs_n, int 
 // observation (pair-interleaved layout of stage_obs).  pix[0..3] = (w_s / sigma_s)^2, pix[4] = gamma_lo, pix[5] = gamma
 // span, pix[6] = gamma_hi; without flags these are the configured values.  Bit 2 (reading S1): pix[7],
 // pix[8] = stored genes (B, gamma) of the centre-of-gravity member, pix[9] = B_los [G]; `off` = sd.off[gd.seed_line].
-#define ME_PIX_WORDS 12
+#define ME_PIX_WORDS 16
 __device__ __forceinline__ void pixel_prologue(const float* obs_s, int L, const GaDesc& gd, float* pix, bool writer,
                                                const float* off = nullptr) {
     const int lane = threadIdx.x & 31;
@@ -673,6 +703,100 @@ __device__ __forceinline__ void pixel_prologue(const float* obs_s, int L, const 
             pix[9] = blos;
         }
     }
+}
+
+// Reading S2: the weak-field member "as in Auer et al. (1977)", prologue bit 8, run like
+// pixel_prologue by every warp on the staged observation; the writer fills pix[10..12] = stored genes (B, gamma, chi) and
+// pix[13] = B_los [G].  pix[4], pix[6] (the pixel's inclination box) must have been written by the same thread before.
+//   B_los from the separation of the I+V and I-V line cores (parabola vertex at the first minimum), chi and gamma from the
+//   maxima of Q^2 + U^2, |V|, |I'|, |I''| on the interior samples of the seed line's window; off = lambda_j - lambda_0.
+__device__ __forceinline__ void pixel_seed_auer(const float* obs_s, int L, const GaDesc& gd, float* pix, bool writer,
+                                                const float* off) {
+    const int lane = threadIdx.x & 31;
+    const float INF = __int_as_float(0x7f800000), hw = gd.seed_hw;
+    const int NONE = 0x7fffffff;
+    float yp = INF, ym = INF, D1 = 0.f, D2 = 0.f, Vm = 0.f, L2m = -1.f;
+    int jp = NONE, jm = NONE, jL = NONE;
+#pragma unroll 1
+    for (int j = lane; j < L; j += 32) {                         // ascending j per lane: strict compares keep the first
+        const float dj = off[j];
+        if (fabsf(dj) > hw) continue;
+        const float* o = obs_s + 8 * (j >> 1) + (j & 1);
+        const float I = o[0], V = o[6];
+        const float a = I + V, b = I - V;
+        if (a < yp) { yp = a; jp = j; }
+        if (b < ym) { ym = b; jm = j; }
+        if (j >= 1 && j + 1 < L && fabsf(off[j - 1]) <= hw && fabsf(off[j + 1]) <= hw) {       // interior sample
+            const float hm = dj - off[j - 1], hp = off[j + 1] - dj;
+            const float Im = obs_s[8 * ((j - 1) >> 1) + ((j - 1) & 1)], Ip = obs_s[8 * ((j + 1) >> 1) + ((j + 1) & 1)];
+            const float d1 = (Ip - Im) / (hm + hp);
+            const float d2 = 2.0f * ((Ip - I) / hp - (I - Im) / hm) / (hm + hp);
+            D1 = fmaxf(D1, fabsf(d1)); D2 = fmaxf(D2, fabsf(d2)); Vm = fmaxf(Vm, fabsf(V));
+            const float l2 = fmaf(o[2], o[2], o[4] * o[4]);
+            if (l2 > L2m) { L2m = l2; jL = j; }
+        }
+    }
+#pragma unroll 1
+    for (int s = 16; s > 0; s >>= 1) {
+        D1 = fmaxf(D1, __shfl_xor_sync(0xffffffffu, D1, s)); D2 = fmaxf(D2, __shfl_xor_sync(0xffffffffu, D2, s));
+        Vm = fmaxf(Vm, __shfl_xor_sync(0xffffffffu, Vm, s));
+        float ov = __shfl_xor_sync(0xffffffffu, yp, s); int oj = __shfl_xor_sync(0xffffffffu, jp, s);
+        if (ov < yp || (ov == yp && oj < jp)) { yp = ov; jp = oj; }
+        ov = __shfl_xor_sync(0xffffffffu, ym, s); oj = __shfl_xor_sync(0xffffffffu, jm, s);
+        if (ov < ym || (ov == ym && oj < jm)) { ym = ov; jm = oj; }
+        ov = __shfl_xor_sync(0xffffffffu, L2m, s); oj = __shfl_xor_sync(0xffffffffu, jL, s);
+        if (ov > L2m || (ov == L2m && oj < jL)) { L2m = ov; jL = oj; }
+    }
+    if (!writer) return;
+    pix[10] = pix[11] = pix[12] = pix[13] = 0.f;
+    if (jp == NONE) return;                                      // empty window
+    auto at = [&](int st, int j) { return obs_s[8 * (j >> 1) + 2 * st + (j & 1)]; };
+    auto interior = [&](int j) { return j >= 1 && j + 1 < L && fabsf(off[j - 1]) <= hw && fabsf(off[j]) <= hw && fabsf(off[j + 1]) <= hw; };
+    float core[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {                                // 1. line cores of I + V (k = 0) and I - V (k = 1)
+        const float sg = k == 0 ? 1.0f : -1.0f, y1 = k == 0 ? yp : ym;
+        const int j = k == 0 ? jp : jm;
+        float x = off[j];
+        if (interior(j)) {                                       // vertex of the parabola through the minimum and its neighbours
+            const float y0 = at(0, j - 1) + sg * at(3, j - 1), y2 = at(0, j + 1) + sg * at(3, j + 1);
+            const float a0 = x - off[j - 1], a2 = x - off[j + 1];
+            const float num = a0 * a0 * (y1 - y2) - a2 * a2 * (y1 - y0), den = a0 * (y1 - y2) - a2 * (y1 - y0);
+            if (den != 0.f) x -= 0.5f * num / den;
+        }
+        core[k] = x;
+    }
+    const float blos = (core[0] - core[1]) * gd.seed_scale;      // seed_scale = 1 / (2 C g lambda0^2)
+    float QL = 0.f, UL = 0.f, d2L = 0.f;                         // 3. azimuth at the maximum of the linear polarisation
+    if (jL != NONE) {
+        const float hm = off[jL] - off[jL - 1], hp = off[jL + 1] - off[jL];
+        d2L = 2.0f * ((at(0, jL + 1) - at(0, jL)) / hp - (at(0, jL) - at(0, jL - 1)) / hm) / (hm + hp);
+        QL = at(1, jL); UL = at(2, jL);
+    } else L2m = 0.f;
+    const float s = d2L >= 0.f ? -1.0f : 1.0f;
+    float chi = 0.5f * atan2f(s * UL, s * QL) * 57.29577951308232f;
+    if (chi < 0.f) chi += 180.0f;
+    if (chi >= 180.0f) chi -= 180.0f;
+    float gp = 90.0f;                                            // 4. inclination from the L / V amplitude ratio
+    if (Vm > 0.f && D2 > 0.f) gp = atanf(2.0f * sqrtf(sqrtf(L2m)) * D1 / (Vm * sqrtf(D2))) * 57.29577951308232f;
+    const float glo = pix[4], ghi = pix[6];
+    float gam = blos >= 0.f ? gp : 180.0f - gp;
+    if (gam < glo || gam > ghi) gam = 180.0f - gam;              // the seed is checked against the polarity box
+    gam = fminf(fmaxf(gam, glo), ghi);
+    const float cg = fmaxf(fabsf(cospif(gam * (1.0f / 180.0f))), 0.125f);      // 5. field strength
+    const float hiB = gd.log_scale[0] ? gd.lo[0] * exp2f(gd.log2ratio[0]) : gd.lo[0] + gd.span[0];
+    const float b = fminf(fmaxf(fabsf(blos) / cg, gd.lo[0]), hiB);
+    float uB = 0.f;
+    if (gd.log_scale[0]) { if (gd.log2ratio[0] != 0.f) uB = log2f(b / gd.lo[0]) / gd.log2ratio[0]; }
+    else if (gd.span[0] != 0.f) uB = (b - gd.lo[0]) / gd.span[0];
+    const float ug = ghi > glo ? (gam - glo) / (ghi - glo) : 0.f;
+    const float chic = fminf(fmaxf(chi, gd.lo[2]), gd.lo[2] + gd.span[2]);
+    const float uc = gd.span[2] > 0.f ? (chic - gd.lo[2]) / gd.span[2] : 0.f;
+    const float q[3] = {rintf(fminf(fmaxf(uB, 0.f), 1.f) * 1023.0f), rintf(fminf(fmaxf(ug, 0.f), 1.f) * 1023.0f),
+                        rintf(fminf(fmaxf(uc, 0.f), 1.f) * 1023.0f)};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) pix[10 + k] = gd.variant ? 64.0f * q[k] : __fdiv_rn(q[k], 1023.0f);
+    pix[13] = blos;
 }
 
 // Block-wide argmin of (value, index) with ties -> lowest index. Values must be >= 0 or +Inf.

@@ -13,34 +13,52 @@ namespace me {
 // nm_s:  shared memory, per wavelength pair one float2 of I_fixed (M = 11 only).
 // ------------------------------------------------------------------------------------------------------------
 // far_s != nullptr (FARS): [2 NL][far_stride] float4 of shared memory, this thread's column.
+// off_s != nullptr: the offsets lambda_j - lambda_l staged pair-wise in shared memory, off_s[jp * NL + l] = (off[l][2jp],
+// off[l][2jp+1]), with one padding pair at the end (stage_offsets); else they are read from the constant bank.
 template <int NL, bool TRIPLET, int M, bool FARS = false>
 __device__ __forceinline__ float fitness_params(const float* p, float mu, const SynthDesc& sd, const GaDesc& gd,
                                                 const float4* obs_s, const float2* nm_s, const float* pix,
-                                                float4* far_s = nullptr, int far_stride = 0) {
+                                                float4* far_s = nullptr, int far_stride = 0, const f2* off_s = nullptr) {
     Individual<NL> ind;
-    setup_individual<NL, M>(ind, p, mu, sd);
-    ind.far_s = far_s; ind.far_stride = far_stride;
+    setup_individual<NL, M>(ind, p, mu, sd, TRIPLET);
+    ind.far_addr = 0; ind.far_stride = 16 * far_stride;
     if (FARS) {
 #pragma unroll
         for (int l = 0; l < NL; ++l) far_store(far_s + 2 * l * far_stride, far_stride, ind.far[l]);
+        ind.far_addr = (unsigned)__cvta_generic_to_shared(far_s);
+        keep_in_register(ind.far_addr);          // else S2R + LEA + moves are re-issued in every far-tier branch (r2c)
     }
     f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
     const int L = sd.L, npair = L >> 1;
-    // the offsets lambda_j - lambda_l of the NEXT pair are loaded one iteration ahead: the indexed constant load otherwise
-    // stalls the first FFMA2 of every line (short scoreboard, profiles/r1e)
+    // the offsets lambda_j - lambda_l of the NEXT pair are loaded one iteration ahead: the load otherwise stalls the first
+    // FFMA2 of every line (profiles/r1_history.md, step r1e).  From shared memory this is one LDS.128 per pair for two lines, and the padding
+    // pair makes the look-ahead of the last iteration a valid read (r2c: the constant-bank form cost 2 LDC + 2 index
+    // instructions per wavelength point).
     f2 offn[NL];
 #pragma unroll
-    for (int l = 0; l < NL; ++l) offn[l] = *reinterpret_cast<const f2*>(&sd.off[l][0]);
+    for (int l = 0; l < NL; ++l) offn[l] = off_s != nullptr ? off_s[l] : *reinterpret_cast<const f2*>(&sd.off[l][0]);
     for (int jp = 0; jp < npair; ++jp) {
         f2 I, Q, U, V, offc[NL];
-        const int jn = 2 * min(jp + 1, npair - 1);
 #pragma unroll
-        for (int l = 0; l < NL; ++l) { offc[l] = offn[l]; offn[l] = *reinterpret_cast<const f2*>(&sd.off[l][jn]); }
-        stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V, offc);
+        for (int l = 0; l < NL; ++l) offc[l] = offn[l];
+        if (off_s != nullptr) {
+            if (NL == 2) {
+                const float4 o = *reinterpret_cast<const float4*>(off_s + 2 * (jp + 1));
+                offn[0] = make_float2(o.x, o.y); offn[NL - 1] = make_float2(o.z, o.w);
+            } else {
+#pragma unroll
+                for (int l = 0; l < NL; ++l) offn[l] = off_s[(jp + 1) * NL + l];
+            }
+        } else {
+            const int jn = 2 * min(jp + 1, npair - 1);
+#pragma unroll
+            for (int l = 0; l < NL; ++l) offn[l] = *reinterpret_cast<const f2*>(&sd.off[l][jn]);
+        }
         const float4 o0 = obs_s[2 * jp], o1 = obs_s[2 * jp + 1];           // (I0,I1,Q0,Q1), (U0,U1,V0,V1)
-        const f2 dI = sub2(make_float2(o0.x, o0.y), I), dQ = sub2(make_float2(o0.z, o0.w), Q);
-        const f2 dU = sub2(make_float2(o1.x, o1.y), U), dV = sub2(make_float2(o1.z, o1.w), V);
-        aI = fma2(dI, dI, aI); aQ = fma2(dQ, dQ, aQ); aU = fma2(dU, dU, aU); aV = fma2(dV, dV, aV);
+        I = make_float2(o0.x, o0.y); Q = make_float2(o0.z, o0.w); U = make_float2(o1.x, o1.y); V = make_float2(o1.z, o1.w);
+        // observed in, residuals observed - model out (stokes_pair RES mode)
+        stokes_pair<NL, TRIPLET, M, FARS, true>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V, offc);
+        aI = fma2(I, I, aI); aQ = fma2(Q, Q, aQ); aU = fma2(U, U, aU); aV = fma2(V, V, aV);
     }
     if (L & 1) {                                                            // odd tail: second half is a duplicate, dropped
         f2 I, Q, U, V;
@@ -61,12 +79,12 @@ __device__ __forceinline__ float fitness_params(const float* p, float mu, const 
 template <int NL, bool TRIPLET, int M, bool FARS = false>
 __device__ __forceinline__ float fitness(const float* g, float mu, const SynthDesc& sd, const GaDesc& gd,
                                          const float4* obs_s, const float2* nm_s, const float* pix,
-                                         float4* far_s = nullptr, int far_stride = 0) {
+                                         float4* far_s = nullptr, int far_stride = 0, const f2* off_s = nullptr) {
     float p[M];
 #pragma unroll
     for (int j = 0; j < M; ++j) p[j] = decode_gene(gene_value(g[j], gd), gd, j);
     if (!gd.log_scale[1]) p[1] = fmaf(pix[5], gene_value(g[1], gd), pix[4]);   // inclination: per-pixel box (reading P1)
-    return fitness_params<NL, TRIPLET, M, FARS>(p, mu, sd, gd, obs_s, nm_s, pix, far_s, far_stride);
+    return fitness_params<NL, TRIPLET, M, FARS>(p, mu, sd, gd, obs_s, nm_s, pix, far_s, far_stride, off_s);
 }
 
 // Stage I_fixed[L] pair-wise: nm_s[jp] = (F[2jp], F[2jp+1]); the odd tail duplicates its single value.
@@ -77,11 +95,24 @@ __device__ __forceinline__ void stage_nm(float2* nm_s, const float* nm, int L, i
     }
 }
 
+// Stage the wavelength offsets pair-wise: off_s[jp * NL + l] = (off[l][2 jp], off[l][2 jp + 1]) for jp < L / 2, plus one padding
+// pair (a copy of the last) that the loop's look-ahead reads.  Same for every pixel: once per CTA.  16-byte aligned for NL = 2.
+template <int NL>
+__device__ __forceinline__ void stage_offsets(f2* off_s, const SynthDesc& sd, int tid, int nthreads) {
+    const int npair = sd.L >> 1;
+    for (int k = tid; k < (npair + 1) * NL; k += nthreads) {
+        const int jp = min(k / NL, max(npair - 1, 0)), l = k % NL;
+        off_s[k] = (NL == ME_MAX_LINES && l >= sd.n_lines) ? make_float2(0.f, 0.f)
+                                                            : make_float2(sd.off[l][2 * jp], sd.off[l][2 * jp + 1]);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // The fused GA inversion kernel.
-// Dynamic shared memory: scratch [64] | pix [8] (per-pixel weights and inclination box) | far [2 NL][THREADS] float4
-//                        (far-tier coefficients of every thread) | obs_s [ceil(L/2)] 2 x float4 |
-//                        nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] | order [pop] u16 (variant 1: ranks at restarts)
+// Dynamic shared memory: scratch [64] | pix [ME_PIX_WORDS] (per-pixel weights and inclination box) | far [2 NL][THREADS] float4
+//                        (far-tier coefficients of every thread) | obs_s [ceil(L/2)] 2 x float4 | off_s [(L/2 + 1) NL] float2
+//                        (wavelength offsets, pair-wise) | nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] |
+//                        order [pop] u16 (variant 1: ranks at restarts)
 // ------------------------------------------------------------------------------------------------------------
 template <int NL, bool TRIPLET, int M, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -96,11 +127,13 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
     constexpr bool FARS = TRIPLET && NL <= 2;                  // far-tier coefficients parked in shared memory
     float4* far_s = reinterpret_cast<float4*>(pix_s + ME_PIX_WORDS) + threadIdx.x;   // [2 NL][THREADS] float4, own column
     float* obs_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? 2 * NL * THREADS : 0));
-    float2* nm_s = reinterpret_cast<float2*>(obs_s + 8 * ((L + 1) >> 1));
+    f2* off_s = reinterpret_cast<f2*>(obs_s + 8 * ((L + 1) >> 1));                     // [(L/2 + 1) NL] float2, 16-byte aligned
+    float2* nm_s = reinterpret_cast<float2*>(off_s + ((L >> 1) + 1) * NL);
     float* genes_s = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));
     float* chi2_s = genes_s + 2 * pop * M;
     uint16_t* order_s = reinterpret_cast<uint16_t*>(chi2_s + 2 * pop);
     if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, threadIdx.x, THREADS);     // once per CTA; synced below
+    stage_offsets<NL>(off_s, sd, threadIdx.x, THREADS);                                // once per CTA; synced below
     const int tid = threadIdx.x;
     const float INF = __int_as_float(0x7f800000);
 
@@ -117,6 +150,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, tid, THREADS);
         __syncthreads();
         pixel_prologue(obs_s, L, gd, pix_s, tid == 0, sd.off[gd.seed_line]);   // every warp reduces, thread 0 writes; visible after the next barrier
+        if (gd.prologue & 8) pixel_seed_auer(obs_s, L, gd, pix_s, tid == 0, sd.off[gd.seed_line]);   // reading S2
 
         // generations 0..G with ONE fitness call site (keeps the loop body inside the instruction cache)
         float g[M];
@@ -145,6 +179,9 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
                         if (tid == pop - 1) g[0] = 0.0f;                              // the non-magnetic solution
                         if (tid == pop - 2) { g[0] = pix_s[7]; g[1] = pix_s[8]; }     // centre-of-gravity longitudinal field
                     }
+                    if ((gd.prologue & 8) && pop >= 4 && tid == pop - 3) {            // reading S2: the Auer weak-field member
+                        g[0] = pix_s[10]; g[1] = pix_s[11]; g[2] = pix_s[12];
+                    }
                 } else if (tid == 0) {
 #pragma unroll
                     for (int j = 0; j < M; ++j) g[j] = gprev[ie * M + j];
@@ -156,7 +193,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
                 } else {
                     make_child<M>(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
                 }
-                if (evaluate) f = fitness<NL, TRIPLET, M, FARS>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s, far_s, THREADS);
+                if (evaluate) f = fitness<NL, TRIPLET, M, FARS>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s, far_s, THREADS, off_s);
 #pragma unroll
                 for (int j = 0; j < M; ++j) gnext[tid * M + j] = g[j];
                 chi2_s[(cur ^ 1) * pop + tid] = f;
@@ -198,6 +235,14 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* tile = reinterpret_cast<float*>(smem4) + warp * (32 * SYNTH_VS);
     const int L = sd.L, npair = L >> 1;
+    // as in the GA kernel (r2c: this kernel still rematerialised the far-tier coefficients with scalar FMULs, 4.4 per
+    // wavelength point against 1.8, and read the offsets with two constant loads per point): coefficients parked in shared
+    // memory, one column per thread, and the wavelength offsets staged pair-wise once per CTA
+    constexpr bool FARS = TRIPLET && NL <= 2;
+    float4* far_s = smem4 + (SYNTH_THREADS / 32) * 32 * SYNTH_VS / 4 + threadIdx.x;        // [2 NL][SYNTH_THREADS] float4, own column
+    f2* off_s = reinterpret_cast<f2*>(far_s - threadIdx.x + (FARS ? 2 * NL * SYNTH_THREADS : 0));   // [(L/2 + 1) NL] float2
+    stage_offsets<NL>(off_s, sd, threadIdx.x, SYNTH_THREADS);
+    __syncthreads();
     const bool want_out = out_stokes != nullptr, want_chi2 = out_chi2 != nullptr;
     for (int64_t base = (int64_t)blockIdx.x * SYNTH_THREADS; base < P; base += (int64_t)gridDim.x * SYNTH_THREADS) {
         const int64_t wbase = base + warp * 32;                 // first vector of this warp
@@ -209,7 +254,14 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
         for (int j = 0; j < M; ++j) p[j] = __ldg(params + v * M + j);
         const float mu = mu_arr != nullptr ? __ldg(mu_arr + v) : 1.0f;
         Individual<NL> ind;
-        setup_individual<NL, M>(ind, p, mu, sd);
+        setup_individual<NL, M>(ind, p, mu, sd, TRIPLET);
+        ind.far_addr = 0; ind.far_stride = 16 * SYNTH_THREADS;
+        if (FARS) {
+#pragma unroll
+            for (int l = 0; l < NL; ++l) far_store(far_s + 2 * l * SYNTH_THREADS, SYNTH_THREADS, ind.far[l]);
+            ind.far_addr = (unsigned)__cvta_generic_to_shared(far_s);
+            keep_in_register(ind.far_addr);
+        }
         const float* nm = sd.nm_profile;
         f2 aI = bc(0.f), aQ = bc(0.f), aU = bc(0.f), aV = bc(0.f);
         for (int jp0 = 0; jp0 < npair; jp0 += SYNTH_CW / 2) {
@@ -218,7 +270,10 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
                 const int j = 2 * (jp0 + i);
                 f2 I, Q, U, V;
                 const f2 nmF = M == ME_MAX_NPAR ? make_float2(__ldg(nm + j), __ldg(nm + j + 1)) : bc(0.f);
-                stokes_pair<NL, TRIPLET, M>(ind, sd, j, false, nmF, I, Q, U, V);
+                f2 offc[NL];
+#pragma unroll
+                for (int l = 0; l < NL; ++l) offc[l] = off_s[(jp0 + i) * NL + l];
+                stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, j, false, nmF, I, Q, U, V, offc);
                 if (want_out) {
                     float2* t = reinterpret_cast<float2*>(tile + lane * SYNTH_VS + 2 * i);
                     t[0] = I; t[SYNTH_CW / 2] = Q; t[SYNTH_CW] = U; t[3 * SYNTH_CW / 2] = V;
@@ -260,7 +315,7 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
         }
         if (L & 1) {                                             // odd tail: one wavelength, written directly
             f2 I, Q, U, V;
-            stokes_pair<NL, TRIPLET, M>(ind, sd, L - 1, true, M == ME_MAX_NPAR ? bc(__ldg(nm + L - 1)) : bc(0.f), I, Q, U, V);
+            stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, L - 1, true, M == ME_MAX_NPAR ? bc(__ldg(nm + L - 1)) : bc(0.f), I, Q, U, V);
             if (want_out && wbase + lane < P) {
                 float* o = out_stokes + v * 4 * (int64_t)L + (L - 1);
                 __stcs(o, I.x); __stcs(o + L, Q.x); __stcs(o + 2 * L, U.x); __stcs(o + 3 * L, V.x);
@@ -281,7 +336,7 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
 // ------------------------------------------------------------------------------------------------------------
 // ga_uncertainty: sigma of every parameter from the curvature of chi2 at the optimum (eq. 26; reading
 // U1 of DESIGN.md).  CTA = pixel.  The 1 + 2 (2M + 2M(M-1)) chi2 evaluations (325 for M = 9) of the central second
-// differences at h = 2^-7 and h/2 are spread over the block and run through the same fused fitness as the GA; thread 0
+// differences at h = 2^-6 and h/2 are spread over the block and run through the same fused fitness as the GA; thread 0
 // then builds the Richardson-extrapolated Hessian and inverts it in FP64 (Gauss-Jordan, partial pivoting; M <= 11).
 // Dynamic shared memory: scratch [64] | pix [8] | obs_s | nm_s | chi2v [n_eval]
 // ------------------------------------------------------------------------------------------------------------
@@ -321,7 +376,7 @@ ga_uncertainty_kernel(const __grid_constant__ SynthDesc sd, const __grid_constan
     float* chi2v = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));
     if (M == ME_MAX_NPAR) stage_nm(nm_s, sd.nm_profile, L, tid, 128);
     const int ne = unc_n_eval(M);
-    const float h = 1.0f / 128.0f;
+    const float h = 1.0f / 64.0f;     // reading U1 (amended in round 2): the FP32 noise on a curvature goes as eps chi2 / h^2
     const float qnan = __int_as_float(0x7fc00000);
     for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
         if (mask != nullptr && mask[n] == 0) {
@@ -453,7 +508,7 @@ static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, con
                                       const float* mu, int64_t N, float* out_params, float* out_chi2, cudaStream_t st) {
     auto k = ga_invert_kernel<NL, TRIPLET, M, THREADS, MINB>;
     const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * M * 4 + (size_t)2 * gd.pop * 4 + 64 * 4 +
-                        (size_t)2 * gd.pop + 16 + ME_PIX_WORDS * 4 +
+                        (size_t)2 * gd.pop + 16 + ME_PIX_WORDS * 4 + (size_t)8 * NL * (sd.L / 2 + 1) +
                         ((TRIPLET && NL <= 2) ? (size_t)2 * NL * THREADS * 16 : 0);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -506,7 +561,14 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
     const int64_t blocks_needed = (P + SYNTH_THREADS - 1) / SYNTH_THREADS;
     const int64_t cap = (int64_t)sms * 4;                            // persistent grid: 4 resident blocks per SM
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
-    const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float);
+    const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float) +
+                        ((ME_INST_TRIPLET && ME_INST_NL <= 2) ? (size_t)2 * ME_INST_NL * SYNTH_THREADS * 16 : 0) +
+                        (size_t)8 * ME_INST_NL * (sd.L / 2 + 1);
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
     me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, perm, P, out_stokes, obs_ref, w2[0],
                                                                                    w2[1], w2[2], w2[3], inv_nu, out_chi2);
     return cudaGetLastError();

@@ -4,7 +4,8 @@
 //   ga_invert_kernel   CTA = one pixel, thread = one individual; the whole GA of Alg. 1 runs
 //                      on-chip: observation staged once in shared memory, population double-buffered in shared
 //                      memory, fitness (synthesis + eq. 16) accumulated in registers over a serial wavelength loop.
-//   me_synth_kernel    warp = one parameter vector, lane = wavelength (coalesced [P,4,L] stores), optional chi2.
+//   me_synth_kernel    thread = one parameter vector (the lanes of a warp sit at the same wavelength, as in the GA kernel),
+//                      [P,4,L] stores through a warp-private transpose tile, optional chi2; persistent grid.
 //   ga_fitness_kernel / ga_step_kernel / ga_init_kernel / philox_kernel / faddeeva_kernel: test hooks.
 //
 // The paper's own mapping (block = individual, thread = wavelength, GA on the host with per-generation PCIe
@@ -20,7 +21,8 @@ namespace me {
 // ------------------------------------------------------------------------------------------------------------
 // One generation from given genes and given fitness (shared: genes [pop][M] | chi2 [pop] | scratch [64]).
 template <int M>
-__global__ void ga_step_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ genes_in,
+__global__ void __launch_bounds__(ME_MAX_POP)    // pop threads per block, up to 1024: at most 64 registers (the 11-gene body took 66)
+ga_step_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ genes_in,
                                const float* __restrict__ chi2_in, int64_t N, int t, float* __restrict__ genes_out) {
     extern __shared__ float4 smem4[];
     const int pop = gd.pop, tid = threadIdx.x;
@@ -76,25 +78,30 @@ __global__ void ga_init_kernel(const __grid_constant__ GaDesc gd, int64_t N, flo
     for (int j = 0; j < M; ++j) genes_out[k * M + j] = g[j];
 }
 
-// The per-pixel prologue alone (one warp per pixel): out[n][9] = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi, B_los, and the
-// stored genes (B, gamma) of the centre-of-gravity member.  off: device copy of lambda_j - lambda_(seed line), or nullptr.
-__global__ void ga_prologue_kernel(const __grid_constant__ GaDesc gd, const float* __restrict__ obs, int64_t N, int L,
-                                   const float* __restrict__ off, float* __restrict__ out) {
+// The per-pixel prologue alone (one warp per pixel): out[n][12] = w_I, w_Q, w_U, w_V, gamma_lo, gamma_hi, B_los (centre of
+// gravity), the stored genes (B, gamma) of the centre-of-gravity member, and the stored genes (B, gamma, chi) of the Auer
+// weak-field member.  The offsets lambda_j - lambda_(seed line) are read from the descriptor in the constant bank.
+__global__ void ga_prologue_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ GaDesc gd,
+                                   const float* __restrict__ obs, int64_t N, float* __restrict__ out) {
     extern __shared__ float4 smem4[];
+    const int L = sd.L;
     float* obs_s = reinterpret_cast<float*>(smem4);
     float* pix_s = obs_s + 8 * ((L + 1) >> 1);
+    const float* off = sd.off[gd.seed_line];
     for (int64_t n = blockIdx.x; n < N; n += gridDim.x) {
         __syncwarp();
         stage_obs(obs_s, obs + n * 4 * (int64_t)L, L, threadIdx.x, 32);
         __syncwarp();
-        if (threadIdx.x == 0) pix_s[7] = pix_s[8] = pix_s[9] = 0.f;
+        if (threadIdx.x == 0) for (int k = 7; k < 14; ++k) pix_s[k] = 0.f;
         __syncwarp();
         pixel_prologue(obs_s, L, gd, pix_s, threadIdx.x == 0, off);
+        if (gd.prologue & 8) pixel_seed_auer(obs_s, L, gd, pix_s, threadIdx.x == 0, off);
         __syncwarp();
-        if (threadIdx.x < 4) out[n * 9 + threadIdx.x] = sqrtf(pix_s[threadIdx.x]) * gd.sigma[threadIdx.x];   // back to w_s
+        if (threadIdx.x < 4) out[n * 12 + threadIdx.x] = sqrtf(pix_s[threadIdx.x]) * gd.sigma[threadIdx.x];   // back to w_s
         if (threadIdx.x == 4) {
-            out[n * 9 + 4] = pix_s[4]; out[n * 9 + 5] = pix_s[6];
-            out[n * 9 + 6] = pix_s[9]; out[n * 9 + 7] = pix_s[7]; out[n * 9 + 8] = pix_s[8];
+            out[n * 12 + 4] = pix_s[4]; out[n * 12 + 5] = pix_s[6];
+            out[n * 12 + 6] = pix_s[9]; out[n * 12 + 7] = pix_s[7]; out[n * 12 + 8] = pix_s[8];
+            out[n * 12 + 9] = pix_s[10]; out[n * 12 + 10] = pix_s[11]; out[n * 12 + 11] = pix_s[12];
         }
     }
 }
@@ -269,20 +276,11 @@ cudaError_t launch_ga_init(const GaDesc& gd, int npar, int64_t N, float* genes_o
     return cudaGetLastError();
 }
 
-cudaError_t launch_ga_prologue(const SynthDesc* sd, const GaDesc& gd, const float* obs, int64_t N, int L, float* out,
-                               cudaStream_t st) {
-    const size_t smem = (size_t)32 * ((L + 1) / 2) + ME_PIX_WORDS * 4;
-    float* off = nullptr;                                    // hook only: a stream-ordered scratch copy of the offsets
-    if (sd != nullptr && (gd.prologue & 4)) {
-        cudaError_t e = cudaMallocAsync(&off, (size_t)L * 4, st);
-        if (e != cudaSuccess) return e;
-        e = cudaMemcpyAsync(off, sd->off[gd.seed_line], (size_t)L * 4, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) return e;
-    }
-    ga_prologue_kernel<<<grid_for(N), 32, smem, st>>>(gd, obs, N, L, off, out);
-    cudaError_t e = cudaGetLastError();
-    if (off != nullptr) { cudaStreamSynchronize(st); cudaFreeAsync(off, st); }   // the host copy source is the caller's stack
-    return e;
+// No allocation, no synchronisation: the kernel reads the offsets of the seed line from the descriptor it is passed.
+cudaError_t launch_ga_prologue(const SynthDesc& sd, const GaDesc& gd, const float* obs, int64_t N, float* out, cudaStream_t st) {
+    const size_t smem = (size_t)32 * ((sd.L + 1) / 2) + ME_PIX_WORDS * 4;
+    ga_prologue_kernel<<<grid_for(N), 32, smem, st>>>(sd, gd, obs, N, out);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_philox(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3, int64_t n,

@@ -23,8 +23,7 @@ cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* 
                          cudaStream_t st);
 cudaError_t launch_philox(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3, int64_t n,
                           uint32_t* out, cudaStream_t st);
-cudaError_t launch_ga_prologue(const SynthDesc* sd, const GaDesc& gd, const float* obs, int64_t N, int L, float* out,
-                               cudaStream_t st);
+cudaError_t launch_ga_prologue(const SynthDesc& sd, const GaDesc& gd, const float* obs, int64_t N, float* out, cudaStream_t st);
 cudaError_t launch_probe(int kind, int iters, int blocks, float* out, cudaStream_t st);
 cudaError_t launch_faddeeva(const float* v, const float* a, int64_t n, float* H, float* F, cudaStream_t st);
 

@@ -1,16 +1,13 @@
 """Measures the ALU roofline denominators on the box (SURVEY.md par. 8(d): MEASURED_PEAKS.json has no FP32 / SFU peak).
 
 `python -m paper_1208_0302_b200.peaks` prints one JSON object: lane-slots/s of each probe of include/me.h's
-me_peak_probe (FFMA, FFMA2, mixes, MUFU), the flop/s they imply, and the SM clock sampled during the run.
+me_peak_probe (FFMA, FFMA2, MUFU), the flop/s they imply, and the SM clock sampled during the run.
 Argument marshalling and CUDA-event timing only; the probes are kernels of libme_b200.so.
 """
 import json
 
-KINDS = {0: ("ffma", 1, 0, 0), 1: ("ffma2", 0, 1, 0), 2: ("ffma2+ffma 1:1", 1, 1, 0), 3: ("mufu", 0, 0, 1),
-         4: ("fmul2", 0, 1, 0), 5: ("ffma2+ffma 2:1", 0.5, 1, 0), 6: ("ffma2+mufu 8:1", 0, 1, 0.125),
-         7: ("ffma2 pair*scalar+scalar", 0, 1, 0), 8: ("ffma2 pair*pair+imm", 0, 1, 0), 9: ("ffma2 pair*scalar+pair", 0, 1, 0),
-         10: ("fadd2", 0, 1, 0)}
-FLOP_PER_SLOT = {0: 2.0, 1: 4.0, 2: 6.0, 3: 0.0, 4: 2.0, 5: 5.0, 6: 4.0, 7: 4.0, 8: 4.0, 9: 4.0, 10: 2.0}
+KINDS = {0: ("ffma", 1, 0, 0), 1: ("ffma2", 0, 1, 0), 3: ("mufu", 0, 0, 1)}
+FLOP_PER_SLOT = {0: 2.0, 1: 4.0, 3: 0.0}
 
 
 def measure(iters=4096, blocks_per_sm=8, repeats=5, kinds=None):

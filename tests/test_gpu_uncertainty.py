@@ -1,11 +1,14 @@
 """GPU parity of ga_uncertainty (eq. 26; reading U1 of DESIGN.md) against the oracle.
 
-Tolerance: the GPU evaluates chi2 in FP32 (relative error ~1e-5), and a second difference at
-h = 2^-7 divides that by h^2 = 6e-5, so a curvature H_jj carries an absolute error ~ 3e-5 chi2 / h^2 ~ 0.5 chi2.  Parameters
-whose curvature is far above that (every well-constrained parameter of a strong-field pixel) agree with the FP64 oracle to a
-few per cent (typically 1e-3); parameters the data do not constrain do not, on either side.  The test therefore compares sigma where the
-oracle's own relative uncertainty sigma_u (in box units) is below 0.05: median deviation < 1 %, 90 % of the entries
-within 5 %; and the NaN/zero conventions."""
+Tolerance: the GPU evaluates chi2 in FP32 (relative error eps ~ 1e-5, the rounding of the synthesised
+profile itself, which no re-association of the sum removes).  A second difference at step h divides that by h^2, the h/2
+level by h^2/4, and the Richardson combination (4 D(h/2) - D(h))/3 adds them: every entry of the Hessian carries a noise
+nu ~ 20 eps chi2 / h^2 (~ 10 at h = 2^-6, chi2 = 13).  A perturbation dH changes [H^-1]_ii by at most |H^-1| |dH| relative, i.e.
+sigma_i by (1/2) M nu / lambda_min(H).  So parameters of a pixel whose Hessian is well conditioned agree with the FP64 oracle
+to a per cent or better, and those of an ill-conditioned pixel (eta0 - dlambdaD - a are nearly degenerate) cannot, on any
+FP32 implementation.  The test asserts the distribution (median deviation < 1 %, 90 % of the entries within 5 %) over the
+entries the data constrain (oracle sigma_u < 0.05 in box units), and for every such entry the bound 1 % + M nu / (2 lambda_min)
+computed from the ORACLE's Hessian; it prints how many pixels that bound leaves meaningful.  And the NaN / zero conventions."""
 import os
 
 import numpy as np
@@ -32,16 +35,29 @@ def dev(a, dtype=np.float32):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
 
 
-def _compare(sig_g, sig_o, cfg, min_frac):
+EPS_CHI2 = 1e-5          # relative error of a binary32 chi2 (the fused-fitness test measures it)
+
+
+def _compare(sig_g, sig_o, hess_o, chi2_o, cfg, min_frac):
     span = cfg["hi"] - cfg["lo"]
-    rel_u = sig_o / np.where(span > 0, span, 1.0)
+    act = span > 0
+    rel_u = sig_o / np.where(act, span, 1.0)
     rel_u[:, 0] = sig_o[:, 0] / 1000.0                        # log-scaled B: judge on sigma_B / 1 kG
     good = np.isfinite(sig_o) & np.isfinite(sig_g) & (rel_u < 0.05) & (sig_o > 0)
     assert good.mean() > min_frac, good.mean()
-    dev_ = np.abs(sig_g[good] / sig_o[good] - 1.0)
-    # [H^-1]_ii mixes in the poorly constrained directions of H (eta0 - dlambdaD - a are nearly degenerate), so a few
-    # entries of an ill-conditioned pixel move by more than the typical 1e-3: judge the distribution, not the maximum
-    assert np.median(dev_) < 0.01 and np.quantile(dev_, 0.9) < 0.05 and np.max(dev_) < 0.5, (np.median(dev_), np.quantile(dev_, 0.9), dev_.max())
+    dev_ = np.abs(sig_g / np.where(sig_o > 0, sig_o, 1.0) - 1.0)
+    assert np.median(dev_[good]) < 0.01 and np.quantile(dev_[good], 0.9) < 0.05, (np.median(dev_[good]), np.quantile(dev_[good], 0.9))
+    # the worst entries: bounded pixel by pixel by the predicted effect of the FP32 noise on the inverse
+    h, M = orc.uncertainty_step(), int(act.sum())
+    tight = 0
+    for n in np.flatnonzero(good.any(axis=1)):
+        lam_min = np.linalg.eigvalsh(hess_o[n][np.ix_(act, act)]).min()
+        nu = 20.0 * EPS_CHI2 * chi2_o[n] / h ** 2
+        bound = 0.01 + 0.5 * M * nu / lam_min if lam_min > 0 else np.inf
+        tight += bound < 0.1
+        assert np.all(dev_[n][good[n]] <= bound), (n, dev_[n][good[n]].max(), bound, lam_min)
+    print("uncertainty parity: %d pixels compared, %d with a predicted bound below 10 %%; worst deviation %.3g"
+          % (good.any(axis=1).sum(), tight, dev_[good].max()))
     return good
 
 
@@ -65,22 +81,24 @@ def test_uncertainty_vs_oracle_at_the_ga_optimum(B, which):
     _, cg2 = B.ga_uncertainty(dev(obs), gp, c["lam"], ld, c["ga"], mu=dev(mu))
     assert float(((cg2 - gc).abs() / gc).max()) < 1e-5
     p64 = p32.astype(np.float64)
-    so, co = orc.uncertainty(obs, p64, c["lam"], ln, c["ga"], mu=mu, threads=NTHREADS)
+    so, co, ho = orc.uncertainty(obs, p64, c["lam"], ln, c["ga"], mu=mu, threads=NTHREADS, want_hessian=True)
     assert np.max(np.abs(cg.cpu().numpy() - co) / co) < 2e-4
     sg = sg.cpu().numpy().astype(np.float64)
     # A GA that stopped short of the minimum (config0 is not converged, SURVEY.md par. 7) leaves many pixels on a slope
     # where the full Hessian is indefinite: eq. 26 then has no answer and BOTH sides say NaN for the pixel.
     fin_g, fin_o = np.isfinite(sg).all(axis=1), np.isfinite(so).all(axis=1)
     assert np.mean(fin_g == fin_o) > 0.9, (fin_g.mean(), fin_o.mean())
-    _compare(sg, so, c["ga"], 0.08)
+    print("%s: eq. 26 has an answer (positive definite Hessian) for %d of %d pixels at the GA optimum in FP64, %d on the GPU"
+          % (which, fin_o.sum(), N, fin_g.sum()))
+    _compare(sg, so, ho, co, c["ga"], 0.08)
     # at the generating truth (the neighbourhood of the true minimum at this noise level) the Hessian is positive
     # definite for nearly every pixel and the well-constrained parameters agree
     t32 = truth.astype(np.float32)
     sg2, _ = B.ga_uncertainty(dev(obs), dev(t32), c["lam"], ld, c["ga"], mu=dev(mu))
-    so2, _ = orc.uncertainty(obs, t32.astype(np.float64), c["lam"], ln, c["ga"], mu=mu, threads=NTHREADS)
+    so2, co2, ho2 = orc.uncertainty(obs, t32.astype(np.float64), c["lam"], ln, c["ga"], mu=mu, threads=NTHREADS, want_hessian=True)
     sg2 = sg2.cpu().numpy().astype(np.float64)
     assert np.mean(np.isfinite(so2).all(axis=1)) > 0.8 and np.mean(np.isfinite(sg2).all(axis=1) == np.isfinite(so2).all(axis=1)) > 0.9
-    good = _compare(sg2, so2, c["ga"], 0.4)
+    good = _compare(sg2, so2, ho2, co2, c["ga"], 0.4)
     assert good[:, [0, 1, 2, 6]].mean() > 0.7                  # B, gamma, chi, v_los of strong-field pixels
 
 
@@ -120,7 +138,8 @@ def test_uncertainty_conventions_and_model11(B):
     clean2 = orc.synth(t2, lam, ln, nm_profile=nm.astype(np.float64), threads=NTHREADS)
     obs2 = (clean2 + W.draw_noise(clean2.shape, 1e-3)).astype(np.float32).astype(np.float64)
     s2, _ = B.ga_uncertainty(dev(obs2), dev(t2), lam, ld, ga2)
-    o2, _ = orc.uncertainty(obs2, t2.astype(np.float32).astype(np.float64), lam, ln, ga2, nm_profile=nm.astype(np.float64), threads=NTHREADS)
+    o2, c2, h2 = orc.uncertainty(obs2, t2.astype(np.float32).astype(np.float64), lam, ln, ga2, nm_profile=nm.astype(np.float64),
+                                 threads=NTHREADS, want_hessian=True)
     s2 = s2.cpu().numpy().astype(np.float64)
     assert np.all(s2[:, [5, 9, 10]] == 0.0) and np.all(o2[:, [5, 9, 10]] == 0.0)
-    _compare(s2, o2, ga2, 0.25)
+    _compare(s2, o2, h2, c2, ga2, 0.25)
