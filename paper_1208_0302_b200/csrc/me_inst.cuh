@@ -226,7 +226,9 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 #define SYNTH_VS (4 * SYNTH_CW + 4)      /* row stride: 16-byte aligned rows for LDS.128 / STG.128 */
 #define SYNTH_THREADS 128
 
-template <int NL, bool TRIPLET, int M>
+// OUT: out_stokes is written (plain tail, transpose tile); !OUT: chi2 only (residual tail, no tile).  One tail per instantiation:
+// with both inlined behind a run-time flag the 11-parameter and 4-line variants spilled.
+template <int NL, bool TRIPLET, int M, bool OUT>
 __global__ void __launch_bounds__(SYNTH_THREADS, 4)
 me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
                 const int* __restrict__ perm, int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
@@ -240,10 +242,16 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
     // memory, one column per thread, and the wavelength offsets staged pair-wise once per CTA
     constexpr bool FARS = TRIPLET && NL <= 2;
     float4* far_s = smem4 + (SYNTH_THREADS / 32) * 32 * SYNTH_VS / 4 + threadIdx.x;        // [2 NL][SYNTH_THREADS] float4, own column
-    f2* off_s = reinterpret_cast<f2*>(far_s - threadIdx.x + (FARS ? 2 * NL * SYNTH_THREADS : 0));   // [(L/2 + 1) NL] float2
+    // ref_s: obs_ref staged like the GA kernel's observation (per pair two float4: (I0,I1,Q0,Q1), (U0,U1,V0,V1)); the chi2 leg
+    // read it with eight scalar global loads per pair before (r2c)
+    float* ref_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? 2 * NL * SYNTH_THREADS : 0));   // [ceil(L/2)] 2 x float4
+    f2* off_s = reinterpret_cast<f2*>(ref_s + 8 * ((L + 1) >> 1));                                         // [(L/2 + 1) NL] float2
+    constexpr bool want_out = OUT;
+    const bool want_chi2 = out_chi2 != nullptr;
     stage_offsets<NL>(off_s, sd, threadIdx.x, SYNTH_THREADS);
+    if (want_chi2) stage_obs(ref_s, obs_ref, L, threadIdx.x, SYNTH_THREADS);
     __syncthreads();
-    const bool want_out = out_stokes != nullptr, want_chi2 = out_chi2 != nullptr;
+    const float4* ref4 = reinterpret_cast<const float4*>(ref_s);
     for (int64_t base = (int64_t)blockIdx.x * SYNTH_THREADS; base < P; base += (int64_t)gridDim.x * SYNTH_THREADS) {
         const int64_t wbase = base + warp * 32;                 // first vector of this warp
         if (wbase >= P) continue;
@@ -270,20 +278,33 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
                 const int j = 2 * (jp0 + i);
                 f2 I, Q, U, V;
                 const f2 nmF = M == ME_MAX_NPAR ? make_float2(__ldg(nm + j), __ldg(nm + j + 1)) : bc(0.f);
-                f2 offc[NL];
+                // more than two lines (the run-time-sized fallback) sits at the register limit: it keeps the round-1 form of the
+                // offsets, read from the constant bank (the staged form spilled there)
+                constexpr bool LEAN = NL > 2;
+                f2 offc[LEAN ? 1 : NL];
+                if constexpr (!LEAN) {
 #pragma unroll
-                for (int l = 0; l < NL; ++l) offc[l] = off_s[(jp0 + i) * NL + l];
-                stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, j, false, nmF, I, Q, U, V, offc);
-                if (want_out) {
+                    for (int l = 0; l < NL; ++l) offc[l] = off_s[(jp0 + i) * NL + l];
+                }
+                const f2* offp = LEAN ? nullptr : offc;
+                if constexpr (!OUT) {                                    // chi2 only: residuals straight out of the tail's FMAs
+                    const float4 o0 = ref4[2 * (jp0 + i)], o1 = ref4[2 * (jp0 + i) + 1];
+                    I = make_float2(o0.x, o0.y); Q = make_float2(o0.z, o0.w); U = make_float2(o1.x, o1.y); V = make_float2(o1.z, o1.w);
+                    stokes_pair<NL, TRIPLET, M, FARS, true>(ind, sd, j, false, nmF, I, Q, U, V, offp);
+                    aI = fma2(I, I, aI); aQ = fma2(Q, Q, aQ); aU = fma2(U, U, aU); aV = fma2(V, V, aV);
+                    continue;
+                } else {
+                stokes_pair<NL, TRIPLET, M, FARS>(ind, sd, j, false, nmF, I, Q, U, V, offp);
+                {
                     float2* t = reinterpret_cast<float2*>(tile + lane * SYNTH_VS + 2 * i);
                     t[0] = I; t[SYNTH_CW / 2] = Q; t[SYNTH_CW] = U; t[3 * SYNTH_CW / 2] = V;
                 }
                 if (want_chi2) {
-                    const f2 dI = sub2(make_float2(__ldg(obs_ref + j), __ldg(obs_ref + j + 1)), I);
-                    const f2 dQ = sub2(make_float2(__ldg(obs_ref + L + j), __ldg(obs_ref + L + j + 1)), Q);
-                    const f2 dU = sub2(make_float2(__ldg(obs_ref + 2 * L + j), __ldg(obs_ref + 2 * L + j + 1)), U);
-                    const f2 dV = sub2(make_float2(__ldg(obs_ref + 3 * L + j), __ldg(obs_ref + 3 * L + j + 1)), V);
+                    const float4 o0 = ref4[2 * (jp0 + i)], o1 = ref4[2 * (jp0 + i) + 1];
+                    const f2 dI = sub2(make_float2(o0.x, o0.y), I), dQ = sub2(make_float2(o0.z, o0.w), Q);
+                    const f2 dU = sub2(make_float2(o1.x, o1.y), U), dV = sub2(make_float2(o1.z, o1.w), V);
                     aI = fma2(dI, dI, aI); aQ = fma2(dQ, dQ, aQ); aU = fma2(dU, dU, aU); aV = fma2(dV, dV, aV);
+                }
                 }
             }
             if (want_out) {
@@ -563,14 +584,14 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
     const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float) +
                         ((ME_INST_TRIPLET && ME_INST_NL <= 2) ? (size_t)2 * ME_INST_NL * SYNTH_THREADS * 16 : 0) +
-                        (size_t)8 * ME_INST_NL * (sd.L / 2 + 1);
+                        (size_t)32 * ((sd.L + 1) / 2) + (size_t)8 * ME_INST_NL * (sd.L / 2 + 1);
+    auto k = out_stokes != nullptr ? me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, true>
+                                   : me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, false>;
     if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M><<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, perm, P, out_stokes, obs_ref, w2[0],
-                                                                                   w2[1], w2[2], w2[3], inv_nu, out_chi2);
+    k<<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, perm, P, out_stokes, obs_ref, w2[0], w2[1], w2[2], w2[3], inv_nu, out_chi2);
     return cudaGetLastError();
 }
 

@@ -121,9 +121,16 @@ def test_me_synth_extremes_and_chi2(B):
     want = np.array([orc.chi2(obs, m, w, sig) for m in model])
     _, chi_a = B.me_synth(dev(p), lam, ld, obs_ref=dev(obs), w_over_sigma=w / sig)
     _, chi_b = B.me_synth(dev(p), lam, ld, obs_ref=dev(obs), w_over_sigma=w / sig, want_stokes=False)
-    assert torch.equal(chi_a, chi_b)
-    got = chi_a.cpu().numpy().astype(np.float64)
-    assert np.max(np.abs(got - want) / want) < 2e-4
+    # The two legs are different instantiations since round 2: with the Stokes output the model is formed and subtracted from
+    # the reference, without it the residual is the last FMA of the Unno-Rachkovsky tail (as in the fused GA fitness).  Both
+    # must meet the fused-fitness tolerance against the oracle, and they differ from each other by
+    # binary32 rounding only.
+    for chi in (chi_a, chi_b):
+        got = chi.cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(got - want) / want) < 2e-4
+    mutual = float(((chi_a - chi_b).abs() / chi_a).max())
+    print("me_synth chi2, with vs without Stokes output: max relative difference %.2e" % mutual)
+    assert mutual < 5e-6                                          # measured 2.3e-7
     assert B.me_synth(dev(p[:0]), lam, ld)[0].shape[0] == 0       # empty input
 
 
