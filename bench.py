@@ -42,6 +42,11 @@ def parse():
                          "steps are touched; the line says what was done")
     ap.add_argument("--n-side", type=int, default=0, help="override the map side (config1: 256, config3: 2048, config4: 512)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--lines", type=int, default=0, choices=[0, 3],
+                    help="3: add a synthetic third line (Fe I 6302.5's pattern at 6302.0 A, as in the parity tests) to exercise the "
+                         "run-time-sized multi-line kernels; a measured variant, not a BASELINE config")
+    ap.add_argument("--pop", type=int, default=0, help="override the GA population of the workload (a measured variant, not a BASELINE config)")
+    ap.add_argument("--generations", type=int, default=-1, help="override the number of generations (likewise)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--aux", action="store_true", help="also run the auxiliary me_synth (config2) legs and saturation trace inside this run")
@@ -58,6 +63,14 @@ def workload(args):
     c, n, side = _workload(args)
     if getattr(args, "zeeman", "triplets") == "full":
         c = dict(c, triplets=False)
+    if getattr(args, "lines", 0) == 3:
+        c = dict(c, name=c["name"] + "_3lines", lines=list(c["lines"]) + [dict(W.FE_6302, lambda0=6302.0)])
+    pop, gens = getattr(args, "pop", 0), getattr(args, "generations", -1)
+    if pop > 0 or gens >= 0:            # same box, weights and noise; the name changes so that no counters entry is mistaken for it
+        ga = c["ga"]
+        pop, gens = pop or ga["pop"], gens if gens >= 0 else ga["generations"]
+        c = dict(c, name="%s_pop%d_g%d" % (c["name"], pop, gens),
+                 ga=W.ga_config(pop, gens, sigma=c["sigma"], b_lo=c["b_range"][0], b_hi=c["b_range"][1], npar=c.get("npar", 9)))
     return c, n, side
 
 
