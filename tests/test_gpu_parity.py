@@ -92,6 +92,7 @@ def test_me_synth_vs_oracle(B, name, lines, triplets, lam, P):
     out = out.cpu().numpy().astype(np.float64)
     cont = (p[:, 7] + mu * p[:, 8])[:, None, None]
     err = np.abs(out - ref) / cont
+    print("forward synthesis: max |dStokes| / I_c = %.2e (north_star bound 2e-5)" % err.max())
     assert err.max() <= 2e-5, (name, err.max(), np.unravel_index(err.argmax(), err.shape))
     # mu = NULL means mu = 1
     out1, _ = B.me_synth(dev(p[:64]), lam, ld)
@@ -110,6 +111,7 @@ def test_me_synth_extremes_and_chi2(B):
     ld = B.line_data_from_workload(c1["lines"], True)
     out, _ = B.me_synth(dev(corners), lam, ld)
     err = np.abs(out.cpu().numpy() - ref) / (corners[:, 7] + corners[:, 8])[:, None, None]
+    print("forward synthesis: max |dStokes| / I_c = %.2e (north_star bound 2e-5)" % err.max())
     assert err.max() <= 2e-5
     zero_b = corners[:, 0] == 0.0
     assert float(out[torch.from_numpy(zero_b).cuda()][:, 1:].abs().max()) == 0.0     # B = 0 => Q = U = V = 0 exactly
@@ -190,6 +192,7 @@ def test_me_synth_large_damping(B):
     ref = orc.synth(p, lam, ln, threads=NTHREADS)
     out, _ = B.me_synth(dev(p), lam, B.line_data_from_workload(c1["lines"], True))
     err = np.abs(out.cpu().numpy() - ref) / (p[:, 7] + p[:, 8])[:, None, None]
+    print("forward synthesis: max |dStokes| / I_c = %.2e (north_star bound 2e-5)" % err.max())
     assert err.max() <= 2e-5, (err.max(), p[np.unravel_index(err.argmax(), err.shape)[0]])
 
 
@@ -226,4 +229,5 @@ def test_me_synth_large_batch_order_is_invisible(B):
     idx = np.arange(0, P, 4000)
     ref = orc.synth(p[idx], lam, oracle_lines(c1["lines"], True), mu=mu[idx], threads=NTHREADS)
     err = np.abs(big.cpu().numpy()[idx] - ref) / (p[idx, 7] + mu[idx] * p[idx, 8])[:, None, None]
+    print("forward synthesis: max |dStokes| / I_c = %.2e (north_star bound 2e-5)" % err.max())
     assert err.max() <= 2e-5
