@@ -87,7 +87,8 @@ int me_synth(const float* params, int64_t P, const float* mu, const double* lamb
 /* The same with an optional caller-provided DEVICE workspace ("no allocation visible to the caller
  * except an optional caller-provided workspace").  With workspace_bytes >= me_synth_workspace_bytes(P) (and that size
  * non-zero) the vectors are visited in the order of a counting sort on a coarse key of (dlambdaD, v_los, B), which keeps the
- * lanes of a warp on the same Voigt tiers; every output stays at its own index and is bit-identical to me_synth's.
+ * lanes of a warp on the same Voigt tiers, and the warps draw their 32-vector tasks from a counter in the workspace instead
+ * of a fixed stride; every output stays at its own index and is bit-identical to me_synth's.
  * workspace = NULL or too small: exactly me_synth.  The workspace is scratch: owned by the caller, 16-byte aligned, not
  * read after the work enqueued by this call has run; it may be reused by later calls on the same stream.
  * me_synth_workspace_bytes returns 0 where sorting does not pay (small P) or is not possible (P >= 2^31). */

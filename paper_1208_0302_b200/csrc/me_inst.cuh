@@ -231,8 +231,9 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 template <int NL, bool TRIPLET, int M, bool OUT>
 __global__ void __launch_bounds__(SYNTH_THREADS, 4)
 me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
-                const int* __restrict__ perm, int64_t P, float* __restrict__ out_stokes, const float* __restrict__ obs_ref,
-                float w2I, float w2Q, float w2U, float w2V, float inv_nu, float* __restrict__ out_chi2) {
+                const int* __restrict__ perm, int* __restrict__ task_counter, int64_t P, float* __restrict__ out_stokes,
+                const float* __restrict__ obs_ref, float w2I, float w2Q, float w2U, float w2V, float inv_nu,
+                float* __restrict__ out_chi2) {
     extern __shared__ float4 smem4[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* tile = reinterpret_cast<float*>(smem4) + warp * (32 * SYNTH_VS);
@@ -252,9 +253,22 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
     if (want_chi2) stage_obs(ref_s, obs_ref, L, threadIdx.x, SYNTH_THREADS);
     __syncthreads();
     const float4* ref4 = reinterpret_cast<const float4*>(ref_s);
-    for (int64_t base = (int64_t)blockIdx.x * SYNTH_THREADS; base < P; base += (int64_t)gridDim.x * SYNTH_THREADS) {
-        const int64_t wbase = base + warp * 32;                 // first vector of this warp
-        if (wbase >= P) continue;
+    // A task = 32 consecutive slots of the processing order, one warp.  Warps share nothing after the staging above, so with
+    // a task counter (the ordered visit of large batches) every warp pulls its next task when it is done with the last one:
+    // r2l's static grid-stride left 18 % of the resident warp slots empty (sm__warps_active 13.2 of 16: 13.2 passes per CTA
+    // at P = 1e6, so a fifth of the CTAs ran a 14th while the others idled, and the cost per task follows the sort key).
+    // Tasks are handed out from the END of the order: the key's leading field is the Doppler width, and wide lines (more
+    // wavelengths in the core tier) are the expensive ones, so the longest tasks start first.
+    const int64_t ntask = (P + 31) >> 5;
+    int64_t task = (int64_t)blockIdx.x * (SYNTH_THREADS / 32) + warp;
+    for (;; task += (int64_t)gridDim.x * (SYNTH_THREADS / 32)) {
+        if (task_counter != nullptr) {
+            int t = 0;
+            if (lane == 0) t = atomicAdd(task_counter, 1);
+            task = __shfl_sync(0xffffffffu, t, 0);
+        }
+        if (task >= ntask) break;
+        const int64_t wbase = (task_counter != nullptr ? ntask - 1 - task : task) << 5;   // first slot of this warp
         const int64_t slot = wbase + lane < P ? wbase + lane : P - 1;   // idle lanes recompute the last vector, never store
         const int64_t v = perm != nullptr ? (int64_t)__ldg(perm + slot) : slot;   // processing order -> vector (synth_order_kernel)
         float p[M];
@@ -311,7 +325,24 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
                 __syncwarp();
                 const int ncol = 2 * nloc;
                 const int64_t nvec = P - wbase < 32 ? P - wbase : 32;
-                if ((L & 3) == 0) {                                  // 16-byte aligned rows: 8 rows per store instruction
+                if ((L & 3) == 0 && nloc == SYNTH_CW / 2 && nvec == 32 && P <= 0xffffffffLL) {
+                    // Full tile (all but the last task and a ragged last chunk): lane -> (Stokes row st, column group q) is
+                    // fixed, only the vector 2 it + (lane >> 4) moves with the iteration, so a store is SHFL (32-bit vector
+                    // index), one IMAD.WIDE for the address, LDS.128 at an immediate offset, STG.128.  The general loop
+                    // below spent 28 instructions per store on 64-bit index arithmetic and predicates (r2r: a quarter
+                    // of the warp instructions of this instantiation).
+                    const int st = (lane >> 2) & 3, q = 4 * (lane & 3), hi = lane >> 4;
+                    const float* trow = tile + hi * SYNTH_VS + st * SYNTH_CW + q;
+                    char* obase = reinterpret_cast<char*>(out_stokes + (int64_t)st * L + 2 * jp0 + q);
+                    const unsigned vbytes = 16u * (unsigned)L;                    // bytes per vector: 4 L floats
+                    const unsigned v32 = (unsigned)v;
+#pragma unroll
+                    for (int it = 0; it < 16; ++it) {
+                        const unsigned vv = __shfl_sync(0xffffffffu, v32, 2 * it + hi);
+                        __stcs(reinterpret_cast<float4*>(obase + (uint64_t)vv * vbytes),
+                               *reinterpret_cast<const float4*>(trow + 2 * it * SYNTH_VS));
+                    }
+                } else if ((L & 3) == 0) {                           // 16-byte aligned rows: 8 rows per store instruction
                     const int q = 4 * (lane & 3);
 #pragma unroll 4
                     for (int it = 0; it < 16; ++it) {
@@ -573,9 +604,9 @@ cudaError_t ME_INST_NAME(launch_uncertainty)(const SynthDesc& sd, const GaDesc& 
     return cudaGetLastError();
 }
 
-cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params, const float* mu, const int* perm, int64_t P,
-                                       float* out_stokes, const float* obs_ref, const float* w2, float inv_nu,
-                                       float* out_chi2, cudaStream_t st) {
+cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params, const float* mu, const int* perm,
+                                       int* task_counter, int64_t P, float* out_stokes, const float* obs_ref, const float* w2,
+                                       float inv_nu, float* out_chi2, cudaStream_t st) {
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -591,7 +622,7 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    k<<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, perm, P, out_stokes, obs_ref, w2[0], w2[1], w2[2], w2[3], inv_nu, out_chi2);
+    k<<<grid, SYNTH_THREADS, smem, st>>>(sd, params, mu, perm, task_counter, P, out_stokes, obs_ref, w2[0], w2[1], w2[2], w2[3], inv_nu, out_chi2);
     return cudaGetLastError();
 }
 

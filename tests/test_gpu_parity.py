@@ -212,7 +212,7 @@ def test_me_synth_large_batch_order_is_invisible(B):
     wos = c1["ga"]["stokes_weight"] / c1["ga"]["sigma"]
     # the ordering scratch is the CALLER's: the library reports its size and allocates nothing itself
     need = B.me_synth_workspace_bytes(P)
-    assert need == (2 * P + 32768) * 4 and B.me_synth_workspace_bytes(399999) == 0 and B.me_synth_workspace_bytes(2 ** 31) == 0
+    assert need == (2 * P + 32768 + 32) * 4 and B.me_synth_workspace_bytes(399999) == 0 and B.me_synth_workspace_bytes(2 ** 31) == 0
     big, chi_big = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos,
                               workspace=torch.empty((need,), dtype=torch.uint8, device="cuda"))
     plain, chi_plain = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos, workspace=False)   # me_synth proper
