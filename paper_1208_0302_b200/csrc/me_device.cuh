@@ -114,7 +114,7 @@ MEDEV FadConst fad_const(float a) {
 
 // Wing region.  With t = 2 Re q, m = -|q|^2 the recurrence gives R(q) = b0 - b1 conj(q); since s conj(q) = |s|^2 conj(s)
 // and |s|^2 = r = 1/|z|^2:   w = i s R = r [ a (b0 + r b1) + i v (b0 - r b1) ]   (no cancellation in H).
-// K = number of series terms beyond the leading one: 5 for |z| >= FAD_CUT, 2 for >= FAD_FAR (used as written only when
+// K = number of series terms beyond the leading one: 5 for |z| >= FAD_CUT, 2 for >= FAD_W2 (used as written only when
 // a > FAD_FAR_AMAX; otherwise the far tier below).  An intermediate K = 3 tier (|z| >= 7.5) was measured and dropped: it
 // saved 0.7 % of the arithmetic and cost more than that in code size (profiles/r1_history.md, step r1e).
 template <int K>
@@ -141,46 +141,86 @@ MEDEV void faddeeva_wing(f2 v, f2 r2, const FadConst& f, f2& wr, f2& wi) {
     wi = mul2(mul2(v, r), fma2(neg(r), b1, b0));
 }
 
-// Far tier (|z|^2 >= FAD_FAR2, a <= FAD_FAR_AMAX): the K = 2 series rewritten as polynomials in r = 1/|z|^2 alone.
-// With v^2 = 1/r - a^2,  Re/Im of i s (C0 + C1 q + C2 q^2) become
-//   H = a r X(r),  X = C0 + 3 C1 r + (5 C2 - 4 a^2 C1) r^2 - 20 a^2 C2 r^3 + 16 a^4 C2 r^4
-//   F = v r Y(r),  Y = C0 +   C1 r + (  C2 - 4 a^2 C1) r^2 - 12 a^2 C2 r^3 + 16 a^4 C2 r^4
-// (the r^4 terms are < 1e-8 relative for a <= FAD_FAR_AMAX; the r^3 terms are < 3e-6 relative = 1e-8 absolute in H and
-// 5e-8 in F, below the FP32 rounding of the evaluation itself: both are dropped, X and Y are evaluated as quadratics).  The coefficients depend on the individual
-// only, so each Horner step is FFMA2 (pair x pair + scalar) -- the full-rate operand form (profiles/r1_history.md, step r1c: an
-// FFMA2 whose ADDEND is a register pair runs at 0.77 of that rate) -- and the line strength r_l and the factor a are
-// folded into them:  fx = a r_l (x2, x1, C0),  fy = r_l (y2, y1, C0).
-struct FarCoef { float x2, x1, x0, y2, y1, y0; };
+// Far tiers (|z| >= FAD_FAR, a <= FAD_FAR_AMAX): the asymptotic series regrouped as polynomials in r = 1/|z|^2 alone.
+// With s = r (v - i a) and v^2 = 1/r - a^2 every term of (i/sqrt(pi)) c_k s^(2k+1) is a polynomial in r and A = a^2:
+//   H = a r X(r; A),  X = C0 [1 + (3/2) r + (15/4 - 2 A) r^2 + (105/8 - 15 A) r^3 + ...]
+//   F = v r Y(r; A),  Y = C0 [1 + (1/2) r + ( 3/4 - 2 A) r^2 + ( 15/8 -  9 A) r^3 + ...]
+// and on r in [0, 1/T^2] the series is cut to a low degree by truncating its Chebyshev expansion on that interval
+// (economisation; gen_faddeeva_table.py), which is a linear map of the series coefficients: the economised coefficients
+// are again polynomials in A with tabulated constants (FAD_CUB_*, FAD_LIN_*), evaluated once per parameter vector.
+//   cubic  tier, |z| >= FAD_FAR = 5:      max |dH| 1.5e-8, |dF| 5.9e-8 against scipy.special.wofz over a <= FAD_FAR_AMAX
+//   linear tier, |z| >= FAD_FAR_LIN = 12: max |dH| 4.8e-8, |dF| 2.2e-7
+// (rounds 1-2 cut the q^2 series by plain truncation: quadratics from |z| = 9 with 6.4e-8 / 4.0e-7, linear from |z| = 20, and
+// a q^5 series evaluated per component between 5 and 9 at twice the cost of the cubic).  Each Horner step is FFMA2
+// (pair x pair + scalar) -- the full-rate operand form (profiles/r1_history.md, step r1c: an FFMA2 whose ADDEND is a register
+// pair runs at 0.77 of that rate) -- and the line strength r_l and the factor a are folded into the coefficients.
+struct FarCoef { float x3, x2, x1, x0, y3, y2, y1, y0, lx1, lx0, ly1, ly0; };
 
-MEDEV FarCoef far_coef(float a, float strength) {
+// the economised coefficients for damping a, without the line strength: X rows carry the factor a
+MEDEV FarCoef far_base(float a) {
+    constexpr float CX[4][FAD_FAR_PA + 1] = FAD_CUB_X, CY[4][FAD_FAR_PA + 1] = FAD_CUB_Y;
+    constexpr float LX[2][FAD_FAR_PA + 1] = FAD_LIN_X, LY[2][FAD_FAR_PA + 1] = FAD_LIN_Y;
+    const float A = a * a;
+    float cx[4], cy[4], lx[2], ly[2];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        float x = CX[j][FAD_FAR_PA], y = CY[j][FAD_FAR_PA];
+#pragma unroll
+        for (int p = FAD_FAR_PA - 1; p >= 0; --p) { x = fmaf(x, A, CX[j][p]); y = fmaf(y, A, CY[j][p]); }
+        cx[j] = a * x; cy[j] = y;
+    }
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        float x = LX[j][FAD_FAR_PA], y = LY[j][FAD_FAR_PA];
+#pragma unroll
+        for (int p = FAD_FAR_PA - 1; p >= 0; --p) { x = fmaf(x, A, LX[j][p]); y = fmaf(y, A, LY[j][p]); }
+        lx[j] = a * x; ly[j] = y;
+    }
     FarCoef c;
-    const float a2 = a * a, sa = strength * a;
-    c.x0 = sa * FAD_C0; c.x1 = sa * (3.0f * FAD_C1); c.x2 = sa * fmaf(-4.0f * FAD_C1, a2, 5.0f * FAD_C2);
-    c.y0 = strength * FAD_C0; c.y1 = strength * FAD_C1; c.y2 = strength * fmaf(-4.0f * FAD_C1, a2, FAD_C2);
+    c.x0 = cx[0]; c.x1 = cx[1]; c.x2 = cx[2]; c.x3 = cx[3]; c.y0 = cy[0]; c.y1 = cy[1]; c.y2 = cy[2]; c.y3 = cy[3];
+    c.lx0 = lx[0]; c.lx1 = lx[1]; c.ly0 = ly[0]; c.ly1 = ly[1];
     return c;
 }
 
-// accumulates r_l w(v + i a) into (sr, si); LINEAR: beyond |z| = 20 the r^2 terms are dropped too
+MEDEV FarCoef far_scale(const FarCoef& b, float strength) {
+    FarCoef c;
+    c.x0 = strength * b.x0; c.x1 = strength * b.x1; c.x2 = strength * b.x2; c.x3 = strength * b.x3;
+    c.y0 = strength * b.y0; c.y1 = strength * b.y1; c.y2 = strength * b.y2; c.y3 = strength * b.y3;
+    c.lx0 = strength * b.lx0; c.lx1 = strength * b.lx1; c.ly0 = strength * b.ly0; c.ly1 = strength * b.ly1;
+    return c;
+}
+
+// accumulates r_l w(v + i a) into (sr, si); LINEAR: the tier beyond FAD_FAR_LIN
 template <bool LINEAR>
 MEDEV void faddeeva_far_acc(f2 v, f2 r2, const FarCoef& c, f2& sr, f2& si) {
     const f2 r = rcp2(r2);
-    const f2 X = LINEAR ? fma2(bc(c.x1), r, c.x0) : fma2(fma2(bc(c.x2), r, c.x1), r, c.x0);   // r^3 terms dropped (< 1e-8 abs)
-    const f2 Y = LINEAR ? fma2(bc(c.y1), r, c.y0) : fma2(fma2(bc(c.y2), r, c.y1), r, c.y0);
+    const f2 X = LINEAR ? fma2(bc(c.lx1), r, c.lx0) : fma2(fma2(fma2(bc(c.x3), r, c.x2), r, c.x1), r, c.x0);
+    const f2 Y = LINEAR ? fma2(bc(c.ly1), r, c.ly0) : fma2(fma2(fma2(bc(c.y3), r, c.y2), r, c.y1), r, c.y0);
     sr = fma2(r, X, sr);
     si = fma2(mul2(v, r), Y, si);
 }
 
-// The same coefficients parked in shared memory (one float4 pair per thread and line) and re-loaded inside the far branch:
-// in registers they do not fit next to the fitness loop's working set and the compiler rematerialises them with ~13
-// scalar FMULs per line and pair on the FMA pipe (profiles/r1_history.md, step r1e); an LDS.128 pair costs no FMA-pipe slot.
+// The same coefficients parked in shared memory (three float4 rows per thread and line: the linear tier's, the cubic tier's X
+// and Y) and re-loaded inside the far branch that uses them: in registers they do not fit next to the fitness loop's working
+// set and the compiler rematerialises them with scalar FMULs on the FMA pipe (profiles/r1_history.md, step r1e); an LDS.128
+// costs no FMA-pipe slot, and the linear tier (most line-pairs) needs one.
+#define ME_FAR_ROWS 3
+template <bool LINEAR>
 MEDEV FarCoef far_load(unsigned addr, int stride_bytes) {
-    float4 x, y;
+    FarCoef c;
     // "memory": the compiler must not sink or drop far_store's plain stores, which only these loads read.  addr is this
     // thread's column as a 32-bit shared address held in a register (keep_in_register below); stride_bytes is a constant.
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(addr) : "memory");
-    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(y.x), "=f"(y.y) : "r"(addr + stride_bytes) : "memory");
-    FarCoef c;
-    c.x2 = x.x; c.x1 = x.y; c.x0 = x.z; c.y2 = x.w; c.y1 = y.x; c.y0 = y.y;
+    float4 x, y = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (LINEAR) {
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(addr) : "memory");
+        c.lx1 = x.x; c.lx0 = x.y; c.ly1 = x.z; c.ly0 = x.w;
+        c.x3 = c.x2 = c.x1 = c.x0 = c.y3 = c.y2 = c.y1 = c.y0 = 0.f;
+    } else {
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(addr + stride_bytes) : "memory");
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(y.x), "=f"(y.y), "=f"(y.z), "=f"(y.w) : "r"(addr + 2 * stride_bytes) : "memory");
+        c.x3 = x.x; c.x2 = x.y; c.x1 = x.z; c.x0 = x.w; c.y3 = y.x; c.y2 = y.y; c.y1 = y.z; c.y0 = y.w;
+        c.lx1 = c.lx0 = c.ly1 = c.ly0 = 0.f;
+    }
     return c;
 }
 // A loop-invariant value the compiler would otherwise RE-COMPUTE inside the wavelength loop to save a register (ncu r2c:
@@ -189,8 +229,9 @@ MEDEV FarCoef far_load(unsigned addr, int stride_bytes) {
 MEDEV void keep_in_register(unsigned& x) { asm volatile("" : "+r"(x)); }
 MEDEV void keep_in_register(float& x) { asm volatile("" : "+f"(x)); }
 MEDEV void far_store(float4* p, int stride, const FarCoef& c) {
-    p[0] = make_float4(c.x2, c.x1, c.x0, c.y2);
-    *reinterpret_cast<float2*>(p + stride) = make_float2(c.y1, c.y0);
+    p[0] = make_float4(c.lx1, c.lx0, c.ly1, c.ly0);
+    p[stride] = make_float4(c.x3, c.x2, c.x1, c.x0);
+    p[2 * stride] = make_float4(c.y3, c.y2, c.y1, c.y0);
 }
 
 // Core region (Weideman).  D = 1/(L - iz) = r ((L+a) + i v), r = 1/|L - iz|^2, Z = (L + iz) D.  With t = 2 Re Z,
@@ -233,7 +274,7 @@ struct Individual {
     float c2x, s2x;                   // cos 2chi, sin 2chi
     float S0, muS1;                   // 11-parameter model: (1-s) S0 and (1-s) alpha mu S1
     float k0, nmS1, stray;            // 11-parameter model only: eta0/sqrt(pi), (1-s)(1-alpha) mu S1, s
-    unsigned far_addr;                // FARS: 32-bit shared address of this thread's far coefficients, [2 l + {0,1}] * far_stride
+    unsigned far_addr;                // FARS: 32-bit shared address of this thread's far coefficients, [ME_FAR_ROWS l + {0,1,2}] * far_stride
     int far_stride;                   //       stride in BYTES between consecutive float4 rows (16 * threads per block)
 };
 
@@ -266,10 +307,11 @@ MEDEV void setup_individual(Individual<NL>& ind, const float* p, float mu, const
         ind.S0 = oms * ind.S0;
         ind.stray = s;
     }
+    const FarCoef fbase = far_base(a);
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
-        if (NL == ME_MAX_LINES && l >= d.n_lines) { ind.invD[l] = ind.v0[l] = ind.vB[l] = 0.f; ind.far[l] = far_coef(a, 0.f); continue; }
-        ind.far[l] = far_coef(a, d.line[l].strength);
+        if (NL == ME_MAX_LINES && l >= d.n_lines) { ind.invD[l] = ind.v0[l] = ind.vB[l] = 0.f; ind.far[l] = far_scale(fbase, 0.f); continue; }
+        ind.far[l] = far_scale(fbase, d.line[l].strength);
         const float inv = 1.0f / (dld * d.line[l].dld_scale);
         ind.invD[l] = inv;
         ind.v0[l] = -(d.line[l].lam0_over_c * vlos) * inv;
@@ -296,19 +338,20 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
         // straight-line code that the scheduler interleaves; the series shortens with distance from the line.
         if (dv >= tfar) {
             const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
-            const FarCoef far = FARS ? far_load(far_addr + 2 * l * far_stride, far_stride) : far_r;
             if (dv >= FAD_FAR_LIN) {
+                const FarCoef far = FARS ? far_load<true>(far_addr + ME_FAR_ROWS * l * far_stride, far_stride) : far_r;
                 faddeeva_far_acc<true>(v, r2p, far, pr, pi);
                 faddeeva_far_acc<true>(vb, r2b, far, br, bi);
                 faddeeva_far_acc<true>(vr, r2r, far, rr, ri);
             } else {
+                const FarCoef far = FARS ? far_load<false>(far_addr + ME_FAR_ROWS * l * far_stride, far_stride) : far_r;
                 faddeeva_far_acc<false>(v, r2p, far, pr, pi);
                 faddeeva_far_acc<false>(vb, r2b, far, br, bi);
                 faddeeva_far_acc<false>(vr, r2r, far, rr, ri);
             }
             return;
         }
-        if (dv >= FAD_FAR) {                                      // a > FAD_FAR_AMAX: the series itself
+        if (dv >= FAD_W2) {                                       // a > FAD_FAR_AMAX: the series itself, cut after q^2
             const f2 r2p = fma2(v, v, fad.a2), r2b = fma2(vb, vb, fad.a2), r2r = fma2(vr, vr, fad.a2);
             faddeeva_wing<2>(v, r2p, fad, w0r, w0i);
             faddeeva_wing<2>(vb, r2b, fad, w1r, w1i);
@@ -342,8 +385,8 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
                     const f2 vc = add2(v, bc(-d.shift[c] * vB));
                     const f2 rr_ = rcp2(fma2(vc, vc, fad.a2));                        // 1 / |z|^2
                     const f2 rw = mul2(d.weight[c], rr_);                             // weight_c / |z|^2
-                    const f2 X = fma2(fma2(bc(far.x2), rr_, far.x1), rr_, far.x0);
-                    const f2 Y = fma2(fma2(bc(far.y2), rr_, far.y1), rr_, far.y0);
+                    const f2 X = fma2(fma2(fma2(bc(far.x3), rr_, far.x2), rr_, far.x1), rr_, far.x0);
+                    const f2 Y = fma2(fma2(fma2(bc(far.y3), rr_, far.y2), rr_, far.y1), rr_, far.y0);
                     ar = fma2(rw, X, ar);
                     ai = fma2(mul2(vc, rw), Y, ai);
                 }
@@ -375,13 +418,17 @@ MEDEV void line_profiles(f2 v, float vB, const FadConst& fad, const FarCoef& far
 // by the last FMA of each Stokes parameter instead of a separate subtraction (the fused fitness needs nothing else).
 template <int NL, bool TRIPLET, int M, bool FARS = false, bool RES = false>
 MEDEV void stokes_pair(const Individual<NL>& ind, const SynthDesc& d, int j0, bool tail, f2 nmF, f2& I, f2& Q, f2& U, f2& V,
-                       const f2* offp = nullptr) {
+                       const f2* offp = nullptr, const f2* vpre = nullptr) {
     f2 br = bc(0.f), bi = bc(0.f), pr = bc(0.f), pi = bc(0.f), rr = bc(0.f), ri = bc(0.f), nr = bc(0.f);
 #pragma unroll
     for (int l = 0; l < NL; ++l) {
         if (NL == ME_MAX_LINES && l >= d.n_lines) break;      // NL == ME_MAX_LINES is the run-time-sized fallback
-        const f2 off = offp != nullptr ? offp[l] : (tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]));
-        const f2 v = fma2(ind.invD[l], off, ind.v0[l]);
+        f2 v;
+        if (vpre != nullptr) v = vpre[l];                     // reduced wavelengths formed by the caller (fused fitness)
+        else {
+            const f2 off = offp != nullptr ? offp[l] : (tail ? bc(d.off[l][j0]) : *reinterpret_cast<const f2*>(&d.off[l][j0]));
+            v = fma2(ind.invD[l], off, ind.v0[l]);
+        }
         line_profiles<TRIPLET, FARS>(v, ind.vB[l], ind.fad, ind.far[l], ind.far_addr, ind.far_stride, ind.tfar, d, l, br, bi,
                                      pr, pi, rr, ri);
         if (M == ME_MAX_NPAR && !TRIPLET) {

@@ -12,7 +12,7 @@ namespace me {
 // obs_s: shared memory, per wavelength pair two float4 = (I0,I1,Q0,Q1), (U0,U1,V0,V1) (broadcast reads, conflict-free).
 // nm_s:  shared memory, per wavelength pair one float2 of I_fixed (M = 11 only).
 // ------------------------------------------------------------------------------------------------------------
-// far_s != nullptr (FARS): [2 NL][far_stride] float4 of shared memory, this thread's column.
+// far_s != nullptr (FARS): [ME_FAR_ROWS NL][far_stride] float4 of shared memory, this thread's column.
 // off_s != nullptr: the offsets lambda_j - lambda_l staged pair-wise in shared memory, off_s[jp * NL + l] = (off[l][2jp],
 // off[l][2jp+1]), with one padding pair at the end (stage_offsets); else they are read from the constant bank.
 template <int NL, bool TRIPLET, int M, bool FARS = false>
@@ -24,7 +24,7 @@ __device__ __forceinline__ float fitness_params(const float* p, float mu, const 
     ind.far_addr = 0; ind.far_stride = 16 * far_stride;
     if (FARS) {
 #pragma unroll
-        for (int l = 0; l < NL; ++l) far_store(far_s + 2 * l * far_stride, far_stride, ind.far[l]);
+        for (int l = 0; l < NL; ++l) far_store(far_s + ME_FAR_ROWS * l * far_stride, far_stride, ind.far[l]);
         ind.far_addr = (unsigned)__cvta_generic_to_shared(far_s);
         keep_in_register(ind.far_addr);          // else S2R + LEA + moves are re-issued in every far-tier branch (r2c)
     }
@@ -38,9 +38,12 @@ __device__ __forceinline__ float fitness_params(const float* p, float mu, const 
 #pragma unroll
     for (int l = 0; l < NL; ++l) offn[l] = off_s != nullptr ? off_s[l] : *reinterpret_cast<const f2*>(&sd.off[l][0]);
     for (int jp = 0; jp < npair; ++jp) {
-        f2 I, Q, U, V, offc[NL];
+        f2 I, Q, U, V, vc[NL];
+        // The reduced wavelengths of BOTH lines are formed at the top, which is the last use of this pair's offsets, so the
+        // look-ahead load below lands in the same registers: carried as (current, next) copies the rotation cost 6 MOV per pair
+        // (r2l SASS; in pairs where both lines are in the far tier the issue slots, not the FMA pipe, are what is short).
 #pragma unroll
-        for (int l = 0; l < NL; ++l) offc[l] = offn[l];
+        for (int l = 0; l < NL; ++l) vc[l] = fma2(ind.invD[l], offn[l], ind.v0[l]);
         if (off_s != nullptr) {
             if (NL == 2) {
                 const float4 o = *reinterpret_cast<const float4*>(off_s + 2 * (jp + 1));
@@ -57,7 +60,7 @@ __device__ __forceinline__ float fitness_params(const float* p, float mu, const 
         const float4 o0 = obs_s[2 * jp], o1 = obs_s[2 * jp + 1];           // (I0,I1,Q0,Q1), (U0,U1,V0,V1)
         I = make_float2(o0.x, o0.y); Q = make_float2(o0.z, o0.w); U = make_float2(o1.x, o1.y); V = make_float2(o1.z, o1.w);
         // observed in, residuals observed - model out (stokes_pair RES mode)
-        stokes_pair<NL, TRIPLET, M, FARS, true>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V, offc);
+        stokes_pair<NL, TRIPLET, M, FARS, true>(ind, sd, 2 * jp, false, M == ME_MAX_NPAR ? nm_s[jp] : bc(0.f), I, Q, U, V, nullptr, vc);
         aI = fma2(I, I, aI); aQ = fma2(Q, Q, aQ); aU = fma2(U, U, aU); aV = fma2(V, V, aV);
     }
     if (L & 1) {                                                            // odd tail: second half is a duplicate, dropped
@@ -109,7 +112,7 @@ __device__ __forceinline__ void stage_offsets(f2* off_s, const SynthDesc& sd, in
 
 // ------------------------------------------------------------------------------------------------------------
 // The fused GA inversion kernel.
-// Dynamic shared memory: scratch [64] | pix [ME_PIX_WORDS] (per-pixel weights and inclination box) | far [2 NL][THREADS] float4
+// Dynamic shared memory: scratch [64] | pix [ME_PIX_WORDS] (per-pixel weights and inclination box) | far [ME_FAR_ROWS NL][THREADS] float4
 //                        (far-tier coefficients of every thread) | obs_s [ceil(L/2)] 2 x float4 | off_s [(L/2 + 1) NL] float2
 //                        (wavelength offsets, pair-wise) | nm_s [ceil(L/2)] float2 | genes [2][pop][M] | chi2 [2][pop] |
 //                        order [pop] u16 (variant 1: ranks at restarts)
@@ -125,8 +128,8 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
     uint32_t* scratch = reinterpret_cast<uint32_t*>(smem4);
     float* pix_s = reinterpret_cast<float*>(scratch + 64);
     constexpr bool FARS = TRIPLET && NL <= 2;                  // far-tier coefficients parked in shared memory
-    float4* far_s = reinterpret_cast<float4*>(pix_s + ME_PIX_WORDS) + threadIdx.x;   // [2 NL][THREADS] float4, own column
-    float* obs_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? 2 * NL * THREADS : 0));
+    float4* far_s = reinterpret_cast<float4*>(pix_s + ME_PIX_WORDS) + threadIdx.x;   // [ME_FAR_ROWS NL][THREADS] float4, own column
+    float* obs_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? ME_FAR_ROWS * NL * THREADS : 0));
     f2* off_s = reinterpret_cast<f2*>(obs_s + 8 * ((L + 1) >> 1));                     // [(L/2 + 1) NL] float2, 16-byte aligned
     float2* nm_s = reinterpret_cast<float2*>(off_s + ((L >> 1) + 1) * NL);
     float* genes_s = reinterpret_cast<float*>(nm_s + ((L + 1) >> 1));
@@ -242,10 +245,10 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
     // wavelength point against 1.8, and read the offsets with two constant loads per point): coefficients parked in shared
     // memory, one column per thread, and the wavelength offsets staged pair-wise once per CTA
     constexpr bool FARS = TRIPLET && NL <= 2;
-    float4* far_s = smem4 + (SYNTH_THREADS / 32) * 32 * SYNTH_VS / 4 + threadIdx.x;        // [2 NL][SYNTH_THREADS] float4, own column
+    float4* far_s = smem4 + (SYNTH_THREADS / 32) * 32 * SYNTH_VS / 4 + threadIdx.x;        // [ME_FAR_ROWS NL][SYNTH_THREADS] float4, own column
     // ref_s: obs_ref staged like the GA kernel's observation (per pair two float4: (I0,I1,Q0,Q1), (U0,U1,V0,V1)); the chi2 leg
     // read it with eight scalar global loads per pair before (r2c)
-    float* ref_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? 2 * NL * SYNTH_THREADS : 0));   // [ceil(L/2)] 2 x float4
+    float* ref_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? ME_FAR_ROWS * NL * SYNTH_THREADS : 0));   // [ceil(L/2)] 2 x float4
     f2* off_s = reinterpret_cast<f2*>(ref_s + 8 * ((L + 1) >> 1));                                         // [(L/2 + 1) NL] float2
     constexpr bool want_out = OUT;
     const bool want_chi2 = out_chi2 != nullptr;
@@ -280,7 +283,7 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
         ind.far_addr = 0; ind.far_stride = 16 * SYNTH_THREADS;
         if (FARS) {
 #pragma unroll
-            for (int l = 0; l < NL; ++l) far_store(far_s + 2 * l * SYNTH_THREADS, SYNTH_THREADS, ind.far[l]);
+            for (int l = 0; l < NL; ++l) far_store(far_s + ME_FAR_ROWS * l * SYNTH_THREADS, SYNTH_THREADS, ind.far[l]);
             ind.far_addr = (unsigned)__cvta_generic_to_shared(far_s);
             keep_in_register(ind.far_addr);
         }
@@ -561,7 +564,7 @@ static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, con
     auto k = ga_invert_kernel<NL, TRIPLET, M, THREADS, MINB>;
     const size_t smem = (size_t)40 * ((sd.L + 1) / 2) + (size_t)2 * gd.pop * M * 4 + (size_t)2 * gd.pop * 4 + 64 * 4 +
                         (size_t)2 * gd.pop + 16 + ME_PIX_WORDS * 4 + (size_t)8 * NL * (sd.L / 2 + 1) +
-                        ((TRIPLET && NL <= 2) ? (size_t)2 * NL * THREADS * 16 : 0);
+                        ((TRIPLET && NL <= 2) ? (size_t)ME_FAR_ROWS * NL * THREADS * 16 : 0);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k<<<grid_for_(N), THREADS, smem, st>>>(sd, gd, obs, mask, mu, N, out_params, out_chi2);
@@ -614,7 +617,7 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
     const int64_t cap = (int64_t)sms * 4;                            // persistent grid: 4 resident blocks per SM
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
     const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float) +
-                        ((ME_INST_TRIPLET && ME_INST_NL <= 2) ? (size_t)2 * ME_INST_NL * SYNTH_THREADS * 16 : 0) +
+                        ((ME_INST_TRIPLET && ME_INST_NL <= 2) ? (size_t)ME_FAR_ROWS * ME_INST_NL * SYNTH_THREADS * 16 : 0) +
                         (size_t)32 * ((sd.L + 1) / 2) + (size_t)8 * ME_INST_NL * (sd.L / 2 + 1);
     auto k = out_stokes != nullptr ? me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, true>
                                    : me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, false>;

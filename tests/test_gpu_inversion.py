@@ -139,8 +139,12 @@ def test_config1_subset_full_parity(B):
 def test_config1_full_size_sampled_parity(B):
     # BASELINE config 1 at FULL size (256 x 256 = 65 536 pixels, L = 128, pop 128, 100 generations), in the launch
     # configuration bench.py times (one ga_invert call over the whole map).  The oracle cannot invert 65 536 pixels in
-    # test time, so (a) four blocks of 8 pixels (first, two interior, ragged last) are inverted by the oracle with the
-    # same global pixel ids and compared one by one, and (b) properties that hold at any size are checked on the map.
+    # test time, so (a) sixteen blocks of 8 pixels (first, fourteen interior, ragged last) are inverted by the oracle with
+    # the same global pixel ids and compared one by one, and (b) properties that hold at any size are checked on the map.
+    # (Round 2: four blocks until the far tiers of the Voigt evaluator were re-derived.  The identical-optimum fraction of
+    # the population is 91.6 % on the 1024 pixels of tests/test_gpu_statistical_parity.py (90.5 % before that change); a
+    # 32-pixel sample has a binomial standard deviation of 5 % around it and came out at 25 of 32, so the sample was made
+    # large enough for the unchanged floor of 0.85 to be a test of the kernel and not of the draw.)
     c1 = W.config1()
     N = c1["n_pixels"]
     truth, obs, ln = make_obs(c1, N, threads=NTHREADS)
@@ -159,7 +163,7 @@ def test_config1_full_size_sampled_parity(B):
     assert np.median(np.abs(gp[strong, 0] - truth[strong, 0]) / truth[strong, 0]) < 0.05
     # (a) sampled pixels against the oracle, same Philox streams (keying by global pixel id)
     same = []
-    for start in (0, 20000, 41234, N - 8):
+    for start in [0] + [4099 + 4367 * k for k in range(14)] + [N - 8]:
         sl = slice(start, start + 8)
         res = orc.ga_invert(obs[sl], c1["lam"], ln, c1["ga"], seed=W.SEED_GA, pixel_base=start, threads=NTHREADS)
         ok = np.abs(gc[sl] - res["chi2"]) <= 2e-4 * res["chi2"]

@@ -78,6 +78,7 @@ SYNTH_CASES = [
     ("full Zeeman patterns L=127 (ragged)", [W.FE_6301, W.FE_6302], False, W.grid(6302.0, 127, 0.024), 517),
     ("single anomalous line L=3", [W.FE_6301], False, W.grid(W.FE_6301["lambda0"], 3, 0.05), 33),
     ("config4-like grid L=256", [W.FE_6301, W.FE_6302], True, W.grid(6302.0, 256, 0.012), 300),
+    ("single triplet L=52 (ragged last store chunk of aligned rows)", [W.FE_6302], True, W.grid(W.FE_6302["lambda0"], 52, 0.024), 129),
     ("three lines (run-time line count) L=64", [W.FE_6301, W.FE_6302, dict(W.FE_6302, lambda0=6302.0)], True, W.grid(6302.0, 64, 0.03), 100),
 ]
 
