@@ -115,13 +115,14 @@ def lit(x):
     return t if ("." in t or "e" in t) else t + ".0"
 
 
-def main():
+def main(path=None):
+    """Writes the header (default: faddeeva_table.h beside this script)."""
     L, a = weideman(N)
     c = [1.0 / math.sqrt(math.pi)]
     for k in range(1, K + 1):
         c.append(c[-1] * (2 * k - 1) / 2.0)
     here = os.path.dirname(os.path.abspath(__file__))
-    with open(os.path.join(here, "faddeeva_table.h"), "w") as fh:
+    with open(path or os.path.join(here, "faddeeva_table.h"), "w") as fh:
         fh.write("// Generated by gen_faddeeva_table.py — do not edit.\n#pragma once\n")
         fh.write("#define FAD_N %d\n#define FAD_K %d\n" % (N, K))
         fh.write("#define FAD_CUT2 %.2ff\n" % (CUT * CUT))
