@@ -196,9 +196,12 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
                 } else {
                     make_child<M>(g, gprev, fprev, pixel, (uint32_t)t, (uint32_t)tid, gd.mut_scale[t], gd);
                 }
-                if (evaluate) f = fitness<NL, TRIPLET, M, FARS>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s, far_s, THREADS, off_s);
+                // the genes go to the next buffer BEFORE the fitness call: nothing reads that buffer until the barrier below, and
+                // the M registers are then free inside the wavelength loop (the far-tier loads are asm with a memory clobber,
+                // across which the compiler does not move this store by itself)
 #pragma unroll
                 for (int j = 0; j < M; ++j) gnext[tid * M + j] = g[j];
+                if (evaluate) f = fitness<NL, TRIPLET, M, FARS>(g, mu, sd, gd, reinterpret_cast<const float4*>(obs_s), nm_s, pix_s, far_s, THREADS, off_s);
                 chi2_s[(cur ^ 1) * pop + tid] = f;
             }
             cur ^= 1;
@@ -208,9 +211,10 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
         float fe; int ie;
         block_argmin(f, tid, scratch, fe, ie);             // reading G5
         if (tid == ie) {
+            const float* gfin = genes_s + cur * pop * M + tid * M;     // the last generation's buffer (cur was flipped after it)
 #pragma unroll
-            for (int j = 0; j < M; ++j) out_params[n * M + j] = decode_gene(gene_value(g[j], gd), gd, j);
-            if (!gd.log_scale[1]) out_params[n * M + 1] = fmaf(pix_s[5], gene_value(g[1], gd), pix_s[4]);
+            for (int j = 0; j < M; ++j) out_params[n * M + j] = decode_gene(gene_value(gfin[j], gd), gd, j);
+            if (!gd.log_scale[1]) out_params[n * M + 1] = fmaf(pix_s[5], gene_value(gfin[1], gd), pix_s[4]);
             out_chi2[n] = f;
         }
     }
@@ -232,7 +236,7 @@ ga_invert_kernel(const __grid_constant__ SynthDesc sd, const __grid_constant__ G
 // OUT: out_stokes is written (plain tail, transpose tile); !OUT: chi2 only (residual tail, no tile).  One tail per instantiation:
 // with both inlined behind a run-time flag the 11-parameter and 4-line variants spilled.
 template <int NL, bool TRIPLET, int M, bool OUT>
-__global__ void __launch_bounds__(SYNTH_THREADS, 4)
+__global__ void __launch_bounds__(SYNTH_THREADS, (!OUT && NL <= 2) ? 5 : 4)    // chi2 only: no transpose tile, 15 KB of shared memory, 5 CTAs per SM (the run-time-sized NL = 4 form would spill 1 KB)
 me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ params, const float* __restrict__ mu_arr,
                 const int* __restrict__ perm, int* __restrict__ task_counter, int64_t P, float* __restrict__ out_stokes,
                 const float* __restrict__ obs_ref, float w2I, float w2Q, float w2U, float w2V, float inv_nu,
@@ -245,7 +249,7 @@ me_synth_kernel(const __grid_constant__ SynthDesc sd, const float* __restrict__ 
     // wavelength point against 1.8, and read the offsets with two constant loads per point): coefficients parked in shared
     // memory, one column per thread, and the wavelength offsets staged pair-wise once per CTA
     constexpr bool FARS = TRIPLET && NL <= 2;
-    float4* far_s = smem4 + (SYNTH_THREADS / 32) * 32 * SYNTH_VS / 4 + threadIdx.x;        // [ME_FAR_ROWS NL][SYNTH_THREADS] float4, own column
+    float4* far_s = smem4 + (OUT ? (SYNTH_THREADS / 32) * 32 * SYNTH_VS / 4 : 0) + threadIdx.x;        // [ME_FAR_ROWS NL][SYNTH_THREADS] float4, own column
     // ref_s: obs_ref staged like the GA kernel's observation (per pair two float4: (I0,I1,Q0,Q1), (U0,U1,V0,V1)); the chi2 leg
     // read it with eight scalar global loads per pair before (r2c)
     float* ref_s = reinterpret_cast<float*>(far_s - threadIdx.x + (FARS ? ME_FAR_ROWS * NL * SYNTH_THREADS : 0));   // [ceil(L/2)] 2 x float4
@@ -571,12 +575,15 @@ static cudaError_t launch_ga_invert_t(const SynthDesc& sd, const GaDesc& gd, con
     return cudaGetLastError();
 }
 
-// (pop -> block size, min blocks/SM) keeps the fitness loop at <= 128 registers/thread where the block allows it.
+// (pop -> block size, min blocks/SM).  64- and 128-thread blocks run at 5 warps per scheduler (96 registers, 60 B of spill
+// stores outside the wavelength loop): since the genes are stored before the fitness call the loop body needs 119 registers
+// unconstrained, and at that baseline the fifth warp wins (+3.5 %; at the 125 of rounds 1-2 it lost to 232 B of spills, and a
+// sixth warp at 80 registers loses again: profiles/r2_experiments.md).  Larger blocks keep <= 128 registers/thread.
 #define ME_DISPATCH_THREADS(FN, ...)                                                                          \
     do {                                                                                                        \
         const int pop_ = gd.pop;                                                                                \
-        if (pop_ <= 64) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 64, 8>(__VA_ARGS__);                  \
-        if (pop_ <= 128) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 128, 4>(__VA_ARGS__);                \
+        if (pop_ <= 64) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 64, 10>(__VA_ARGS__);                  \
+        if (pop_ <= 128) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 128, 5>(__VA_ARGS__);                \
         if (pop_ <= 256) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 256, 2>(__VA_ARGS__);                \
         if (pop_ <= 512) return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 512, 1>(__VA_ARGS__);                \
         return FN<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, 1024, 1>(__VA_ARGS__);                                \
@@ -614,9 +621,9 @@ cudaError_t ME_INST_NAME(launch_synth)(const SynthDesc& sd, const float* params,
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int64_t blocks_needed = (P + SYNTH_THREADS - 1) / SYNTH_THREADS;
-    const int64_t cap = (int64_t)sms * 4;                            // persistent grid: 4 resident blocks per SM
+    const int64_t cap = (int64_t)sms * ((out_stokes == nullptr && ME_INST_NL <= 2) ? 5 : 4);   // persistent grid: the resident blocks per SM
     const unsigned grid = (unsigned)(blocks_needed < cap ? blocks_needed : cap);
-    const size_t smem = (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float) +
+    const size_t smem = (out_stokes != nullptr ? (size_t)(SYNTH_THREADS / 32) * 32 * SYNTH_VS * sizeof(float) : 0) +
                         ((ME_INST_TRIPLET && ME_INST_NL <= 2) ? (size_t)ME_FAR_ROWS * ME_INST_NL * SYNTH_THREADS * 16 : 0) +
                         (size_t)32 * ((sd.L + 1) / 2) + (size_t)8 * ME_INST_NL * (sd.L / 2 + 1);
     auto k = out_stokes != nullptr ? me_synth_kernel<ME_INST_NL, ME_INST_TRIPLET, ME_INST_M, true>
