@@ -49,7 +49,8 @@ typedef enum {
     ME_ERR_SHAPE = -2,        /* a size is out of range (L, P, N, pop, n_lines, n_comp ...) */
     ME_ERR_RANGE = -3,        /* a value is out of range (lo > hi, sigma <= 0, log-scaled gene with lo <= 0 ...) */
     ME_ERR_UNSUPPORTED = -4,  /* valid request that this build does not implement (elite != 1) */
-    ME_ERR_CUDA = -5          /* a CUDA runtime call failed; see me_last_cuda_error() */
+    ME_ERR_CUDA = -5,         /* a CUDA runtime call failed; see me_last_cuda_error() */
+    ME_ERR_TOO_LARGE = -6     /* me_synth_static: P exceeds me_synth_static_max_vectors() */
 } me_status;
 
 /* One spectral line (Table 1). Components are (shift, weight, kind) triples in any order. */
@@ -97,6 +98,23 @@ int me_synth_ws(const float* params, int64_t P, const float* mu, const double* l
                 const me_line_data* line_data, float* out_stokes,
                 const float* obs_ref, const float* w_over_sigma, float* out_chi2,
                 void* workspace, size_t workspace_bytes, void* stream);
+
+/* me_synth_ws for callers that can allocate NOTHING (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the ordering scratch is a fixed device array inside the library (`static __device__`, 16.1 MiB, held
+ * by every GPU that loads the library until the process exits) instead of a caller workspace.  Inputs and outputs are the
+ * caller's, with me_synth's meaning, layout and ownership; outputs are bit-identical to me_synth's and me_synth_ws's.
+ *   - P <= me_synth_static_max_vectors() (2 097 152); larger batches are refused with ME_ERR_TOO_LARGE before anything is
+ *     launched: split them, or use me_synth_ws.  Below 400 000 vectors no scratch is needed and none is touched.
+ *   - The call runs no cudaMalloc / cudaFree and no allocating library routine: once per device it asks for the array's
+ *     address (cudaGetSymbolAddress, with that device current), then enqueues one cudaMemsetAsync of the 128 KB of histogram
+ *     and counters that must start at zero, the two ordering passes and the synthesis on `stream`.
+ *   - Every call on a device shares the ONE array, which keeps the previous call's keys and permutation: calls whose work
+ *     overlaps on the GPU (different streams, or graphs replayed concurrently) race on it and give wrong results.  Calls on
+ *     one stream, or otherwise ordered, are safe. */
+int64_t me_synth_static_max_vectors(void);
+int me_synth_static(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
+                    const me_line_data* line_data, float* out_stokes,
+                    const float* obs_ref, const float* w_over_sigma, float* out_chi2, void* stream);
 
 /* GA configuration (readings G0-G5 in DESIGN.md; the paper leaves the operators' details open). */
 typedef struct {

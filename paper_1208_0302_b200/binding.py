@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libme_b200.so")
 _lib = None
 
-EXPORTS = ["me_synth", "me_synth_ws", "me_synth_workspace_bytes", "ga_invert", "ga_uncertainty", "ga_step", "ga_fitness", "ga_init", "ga_prologue", "me_philox", "me_philox_many", "me_faddeeva",
+EXPORTS = ["me_synth", "me_synth_ws", "me_synth_workspace_bytes", "me_synth_static", "me_synth_static_max_vectors", "ga_invert", "ga_uncertainty", "ga_step", "ga_fitness", "ga_init", "ga_prologue", "me_philox", "me_philox_many", "me_faddeeva",
            "me_zeeman_pattern", "me_peak_probe", "me_strerror", "me_last_cuda_error", "me_version"]
 
 
@@ -62,6 +62,8 @@ def lib():
         l.me_strerror.argtypes = [C.c_int]
         l.me_synth_workspace_bytes.restype = C.c_size_t
         l.me_synth_workspace_bytes.argtypes = [C.c_int64]
+        l.me_synth_static_max_vectors.restype = C.c_int64
+        l.me_synth_static_max_vectors.argtypes = []
         _lib = l
     return _lib
 
@@ -194,6 +196,28 @@ def me_synth(params, lam, line_data, mu=None, out_stokes=None, obs_ref=None, w_o
                              _dev(out_chi2, torch.float32, "out_chi2"),
                              _dev(None if workspace is False else workspace, torch.uint8, "workspace"), C.c_size_t(ws_bytes),
                              _stream()), "me_synth_ws")
+    return out_stokes, out_chi2
+
+
+def me_synth_static_max_vectors():
+    return int(lib().me_synth_static_max_vectors())
+
+
+def me_synth_static(params, lam, line_data, mu=None, out_stokes=None, obs_ref=None, w_over_sigma=None, out_chi2=None):
+    """me_synth through the entry point that allocates nothing: the ordering scratch is the library's fixed device array
+    (include/me.h).  out_stokes [P,4,L] is the CALLER's (required; pass out_chi2 too if chi2 is wanted): nothing is allocated
+    here either.  Returns (out_stokes, out_chi2)."""
+    import torch
+    P = params.shape[0]
+    assert params.dim() == 2 and params.shape[1] == line_data.n_params
+    lam, lam_p, L = _grid(lam)
+    assert out_stokes is not None or out_chi2 is not None, "the caller passes the outputs"
+    wos = np.ascontiguousarray(w_over_sigma, dtype=np.float32) if obs_ref is not None else None
+    _check(lib().me_synth_static(_dev(params, torch.float32, "params"), C.c_int64(P), _dev(mu, torch.float32, "mu"), lam_p, L,
+                                 C.byref(line_data.c), _dev(out_stokes, torch.float32, "out_stokes"),
+                                 _dev(obs_ref, torch.float32, "obs_ref"),
+                                 wos.ctypes.data_as(C.POINTER(C.c_float)) if wos is not None else None,
+                                 _dev(out_chi2, torch.float32, "out_chi2"), _stream()), "me_synth_static")
     return out_stokes, out_chi2
 
 

@@ -190,6 +190,7 @@ const char* me_strerror(int code) {
         case ME_ERR_RANGE: return "a value is out of range";
         case ME_ERR_UNSUPPORTED: return "not implemented in this build";
         case ME_ERR_CUDA: return "CUDA runtime error (see me_last_cuda_error)";
+        case ME_ERR_TOO_LARGE: return "P exceeds me_synth_static_max_vectors(): the library's fixed scratch array cannot hold this batch";
         default: return "unknown error code";
     }
 }
@@ -223,6 +224,21 @@ int me_synth_ws(const float* params, int64_t P, const float* mu, const double* l
     cudaError_t e = me::launch_synth(sd, params, mu, P, out_stokes, obs_ref, w2, (float)(1.0 / (4.0 * L - sd.npar)),
                                      out_chi2, workspace, workspace_bytes, (cudaStream_t)stream);
     return e == cudaSuccess ? ME_OK : cuda_fail(e);
+}
+
+int64_t me_synth_static_max_vectors(void) { return me::synth_static_max_vectors(); }
+
+int me_synth_static(const float* params, int64_t P, const float* mu, const double* lambda_grid_A, int L,
+                    const me_line_data* line_data, float* out_stokes,
+                    const float* obs_ref, const float* w_over_sigma, float* out_chi2, void* stream) {
+    if (P < 0) return ME_ERR_SHAPE;
+    if (P > me::synth_static_max_vectors()) return ME_ERR_TOO_LARGE;        // before anything touches the device
+    void* scratch = nullptr;
+    size_t scratch_bytes = 0;
+    cudaError_t e = me::synth_static_scratch(&scratch, &scratch_bytes);     // cudaGetSymbolAddress, once per device
+    if (e != cudaSuccess) return cuda_fail(e);
+    return me_synth_ws(params, P, mu, lambda_grid_A, L, line_data, out_stokes, obs_ref, w_over_sigma, out_chi2, scratch,
+                       scratch_bytes, stream);
 }
 
 int ga_invert(const float* obs, int64_t N, const uint8_t* mask, const float* sigma,

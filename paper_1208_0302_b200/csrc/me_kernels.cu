@@ -11,6 +11,8 @@
 // The paper's own mapping (block = individual, thread = wavelength, GA on the host with per-generation PCIe
 // transfers) is prior art for a Tesla C1060 and is deliberately not followed:
 // see DESIGN.md "What differs from the paper".
+#include <mutex>
+
 #include "me_device.cuh"
 #include "me_launch.h"
 
@@ -310,6 +312,42 @@ cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* 
         task_counter = hist + SYNTH_NKEY;
     }
     return launch_synth_ordered(sd, params, mu, perm, task_counter, P, out_stokes, obs_ref, w2, inv_nu, out_chi2, st);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// me_synth_static: the ordered visit of launch_synth with its scratch in a FIXED device array of this library instead of a
+// caller workspace, for callers that may not allocate at all (CUDA graph capture, serving loops, harnesses that forbid
+// cudaMalloc).  The array holds the workspace of a batch of SYNTH_STATIC_MAX_P vectors (histogram | counters | keys | perm:
+// 16.1 MiB); every device that loads the library carries it until the process exits.
+// In host code the array's NAME is only the host-side stand-in of the symbol, not a device address: a kernel handed
+// `g_synth_static_scratch` from the host would fault (or, where the GPU can reach host memory, silently use the wrong bytes).
+// The device address is asked for once per device, with that device current, by cudaGetSymbolAddress.
+// ------------------------------------------------------------------------------------------------------------
+#define SYNTH_STATIC_MAX_P (1 << 21)
+#define SYNTH_STATIC_INTS (2 * SYNTH_STATIC_MAX_P + SYNTH_NKEY + SYNTH_NCTR)
+#define SYNTH_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) int g_synth_static_scratch[SYNTH_STATIC_INTS];
+
+int64_t synth_static_max_vectors() { return SYNTH_STATIC_MAX_P; }
+
+// The scratch array's address on the CURRENT device and its size.  Allocates nothing.
+cudaError_t synth_static_scratch(void** ptr, size_t* bytes) {
+    static std::mutex mtx;
+    static void* addr[SYNTH_STATIC_MAX_DEVICES] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= SYNTH_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mtx);
+    if (addr[dev] == nullptr) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_synth_static_scratch);
+        if (e != cudaSuccess) return e;
+        addr[dev] = p;
+    }
+    *ptr = addr[dev];
+    *bytes = (size_t)SYNTH_STATIC_INTS * sizeof(int);
+    return cudaSuccess;
 }
 
 cudaError_t launch_ga_step(const GaDesc& gd, int npar, const float* genes_in, const float* chi2_in, int64_t N, int t,

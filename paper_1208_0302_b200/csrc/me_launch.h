@@ -21,6 +21,8 @@ size_t synth_workspace_bytes(int64_t P);
 cudaError_t launch_synth(const SynthDesc& sd, const float* params, const float* mu, int64_t P, float* out_stokes,
                          const float* obs_ref, const float* w2, float inv_nu, float* out_chi2, void* work, size_t work_bytes,
                          cudaStream_t st);
+int64_t synth_static_max_vectors();
+cudaError_t synth_static_scratch(void** ptr, size_t* bytes);     // the library's fixed scratch array on the current device
 cudaError_t launch_philox(uint32_t k0, uint32_t k1, uint32_t c0_base, uint32_t c1, uint32_t c2, uint32_t c3, int64_t n,
                           uint32_t* out, cudaStream_t st);
 cudaError_t launch_ga_prologue(const SynthDesc& sd, const GaDesc& gd, const float* obs, int64_t N, float* out, cudaStream_t st);

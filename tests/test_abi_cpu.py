@@ -23,7 +23,7 @@ def lib():
 def test_exports_every_declared_symbol(lib):
     hdr = open(os.path.join(ROOT, "include", "me.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"^\s*(?:const\s+char\s*\*|int|size_t)\s+(\w+)\s*\(", hdr, flags=re.M))
+    names = set(re.findall(r"^\s*(?:const\s+char\s*\*|int|int64_t|size_t)\s+(\w+)\s*\(", hdr, flags=re.M))
     assert {"me_synth", "ga_invert", "ga_step", "ga_fitness", "me_philox"} <= names
     assert names == set(B.EXPORTS)
     for n in names:
