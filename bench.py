@@ -600,7 +600,7 @@ def run_config2(args):
     roof = roofline_from_counters(key, "me_synth_kernel", P * L, P, launch_s, peak, sm_max, clocks, probe, nbytes)
     roof["hbm"] = {"achieved_gbs": nbytes / launch_s / 1e9, "peak_gbs_measured": float(peaks.get("hbm_gbs", 0.0)) or None,
                    "frac": (nbytes / launch_s / 1e9 / float(peaks["hbm_gbs"])) if peaks.get("hbm_gbs") else None}
-    n_launch = (4 if need else 1)
+    n_launch = (3 if need else 1)    # kernels per me_synth_ws call: histogram + scan, scatter, synthesis (plus one cudaMemsetAsync of 128 KB)
     line = {"metric": "ME syntheses/s", "value": P / launch_s, "unit": "syntheses/s", "n_gpus": 1, "steps": args.steps,
             "warmup": max(args.warmup, 1), "ms_per_step": launch_s * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
