@@ -222,6 +222,14 @@ def test_me_synth_large_batch_order_is_invisible(B):
                                   workspace=torch.empty((need - 16,), dtype=torch.uint8, device="cuda"))   # too small: ignored
     assert torch.equal(big, short) and torch.equal(chi_big, chi_short)
     del plain, short
+    # the chi2-only instantiation (no [P,4,L] output, no transpose tile, 5 CTAs per SM), ordered and in index order: the fused
+    # residual of its tail rounds like the explicit subtraction of the output instantiation or differs by an ulp of chi2
+    for ws in (None, False):
+        _, chi_only = B.me_synth(d_p, lam, ld, mu=d_mu, obs_ref=obs_ref, w_over_sigma=wos, want_stokes=False, workspace=ws)
+        assert torch.allclose(chi_only, chi_big, rtol=2e-4, atol=0.0)
+        if ws is None:
+            chi_only_ordered = chi_only
+    assert torch.equal(chi_only, chi_only_ordered)
     for s in (0, 150000, 300000):
         e = min(s + 150000, P)
         small, chi_small = B.me_synth(d_p[s:e].contiguous(), lam, ld, mu=d_mu[s:e].contiguous(), obs_ref=obs_ref, w_over_sigma=wos)
