@@ -76,6 +76,28 @@ def test_static_scratch_entry_point_matches_existing_paths_twice(B):
     assert torch.equal(chi, chi_plain)
 
 
+def test_static_scratch_entry_point_at_its_maximum_size(B):
+    # exactly me_synth_static_max_vectors() vectors: the batch whose workspace fills the fixed array to its last int (chi2-only
+    # form: a [P,4,L] output of that batch would be 4.3 GB); and P = 0 is a no-op that touches nothing
+    c1 = W.config1()
+    lam = c1["lam"]
+    ld = B.line_data_from_workload(c1["lines"], True)
+    wos = c1["ga"]["stokes_weight"] / c1["ga"]["sigma"]
+    p0, mu0 = _batch(1, 5)
+    obs_ref = B.me_synth(p0, lam, ld, mu=mu0)[0][0].contiguous()
+    P = B.me_synth_static_max_vectors()
+    assert B.me_synth_workspace_bytes(P) == (2 * P + 32768 + 32) * 4          # = the array's size (include/me.h: 16.1 MiB)
+    rng = np.random.default_rng(94)
+    base = W.draw_truth(4096, seed=94, b_lo=1.0, b_hi=3500.0)
+    d_p = dev(base[rng.integers(0, 4096, P)])                                  # 2 097 152 vectors drawn from 4096 distinct ones
+    chi = torch.full((P,), float("nan"), dtype=torch.float32, device="cuda")
+    B.me_synth_static(d_p, lam, ld, obs_ref=obs_ref, w_over_sigma=wos, out_chi2=chi)
+    _, chi_ws = B.me_synth(d_p, lam, ld, obs_ref=obs_ref, w_over_sigma=wos, want_stokes=False)
+    assert torch.equal(chi, chi_ws) and torch.isfinite(chi).all()
+    empty = torch.empty((0, 9), dtype=torch.float32, device="cuda")
+    B.me_synth_static(empty, lam, ld, obs_ref=obs_ref, w_over_sigma=wos, out_chi2=torch.empty((0,), dtype=torch.float32, device="cuda"))
+
+
 def test_static_scratch_entry_point_refuses_batches_beyond_its_array(B):
     lib = B.lib()
     pmax = B.me_synth_static_max_vectors()
